@@ -1,0 +1,185 @@
+"""ctypes front-end of the CPU oracle (oracle/tpc_oracle.cpp).  TEST INFRASTRUCTURE, not the product.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / ``--impl reference`` legs may import
+this package.  It never imports the CUDA package and shares no code with it.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "tpc_oracle.cpp")
+_LIB = os.path.join(_HERE, "libtpcoracle.so")
+
+
+class Params(ctypes.Structure):
+    """DESIGN.md 'Constants' (defaults via oracle_default_params)."""
+    _fields_ = [
+        ("err2_y", ctypes.c_double), ("err2_z", ctypes.c_double),
+        ("nf_ty", ctypes.c_double), ("nf_tz", ctypes.c_double), ("nf_c", ctypes.c_double),
+        ("nf_d2max", ctypes.c_double),
+        ("kf_css0", ctypes.c_double), ("kf_ctt0", ctypes.c_double), ("kf_ckk0", ctypes.c_double),
+        ("kf_smax", ctypes.c_double), ("road_nsig", ctypes.c_double), ("road_max", ctypes.c_double),
+        ("max_gap", ctypes.c_int32), ("min_hits", ctypes.c_int32), ("seed_min_chain", ctypes.c_int32),
+        ("pad", ctypes.c_int32),
+    ]
+
+
+TRACKLET_DTYPE = np.dtype([
+    ("start_gid", np.int64), ("sector", np.int32), ("start_row", np.int32), ("n_hits", np.int32),
+    ("first_row", np.int32), ("last_row", np.int32), ("kept", np.int32), ("n_fit", np.int32),
+    ("near_tie", np.int32), ("x", np.float64), ("p", np.float64, 5), ("c", np.float64, 15),
+    ("chi2", np.float64)], align=True)
+TRACK_DTYPE = np.dtype([
+    ("start_gid", np.int64), ("cluster_offset", np.int64), ("sector", np.int32), ("n_clusters", np.int32),
+    ("first_row", np.int32), ("last_row", np.int32), ("n_fit", np.int32), ("pad", np.int32),
+    ("x", np.float64), ("p", np.float64, 5), ("c", np.float64, 15), ("chi2", np.float64)], align=True)
+
+
+def build(force: bool = False) -> str:
+    """g++ -O2 -ffp-contract=off (IEEE fp32/fp64, no FMA contraction: DESIGN.md R-12)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(["g++", "-O2", "-std=c++17", "-ffp-contract=off", "-fPIC", "-shared",
+                               "-Wall", "-o", _LIB, _SRC])
+    return _LIB
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = ctypes.CDLL(build())
+        vp, i32, i64, dbl = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_double
+        L.oracle_default_params.argtypes = [ctypes.POINTER(Params)]
+        L.oracle_create.restype = vp
+        L.oracle_create.argtypes = [i32, i32, vp, dbl, ctypes.POINTER(Params), i32]
+        L.oracle_destroy.argtypes = [vp]
+        L.oracle_run.argtypes = [vp, vp, vp, vp, i32]
+        for name in ("oracle_n_clusters", "oracle_n_start_hits", "oracle_n_tracklets", "oracle_n_tracks",
+                     "oracle_n_cluster_ids"):
+            getattr(L, name).restype = i64
+            getattr(L, name).argtypes = [vp]
+        L.oracle_get_links.argtypes = [vp, i32, vp]
+        L.oracle_get_tie_flags.argtypes = [vp, vp]
+        L.oracle_get_start_hits.argtypes = [vp, vp]
+        L.oracle_get_tracklets.argtypes = [vp, vp, vp]
+        L.oracle_get_owners.argtypes = [vp, vp]
+        L.oracle_get_tracks.argtypes = [vp, vp, vp]
+        L.oracle_get_stage_seconds.argtypes = [vp, vp]
+        L.oracle_sizeof_tracklet.restype = i32
+        L.oracle_sizeof_track.restype = i32
+        L.oracle_propagate.restype = i32
+        L.oracle_propagate.argtypes = [i32, vp, vp, vp, dbl, dbl, dbl, vp]
+        L.oracle_update.argtypes = [i32, vp, vp, vp, i32, dbl, dbl]
+        assert L.oracle_sizeof_tracklet() == TRACKLET_DTYPE.itemsize, (L.oracle_sizeof_tracklet(), TRACKLET_DTYPE.itemsize)
+        assert L.oracle_sizeof_track() == TRACK_DTYPE.itemsize, (L.oracle_sizeof_track(), TRACK_DTYPE.itemsize)
+        _lib = L
+    return _lib
+
+
+def default_params() -> Params:
+    p = Params()
+    lib().oracle_default_params(ctypes.byref(p))
+    return p
+
+
+class Result:
+    """All stage outputs of one oracle run, in canonical (order-independent) form.
+
+    links: row-local LOAD index of the linked hit in row r+1 (up) / r-1 (down), -1 none, indexed by
+    event-global cluster id.  tracklets/tracks are keyed by ``start_gid`` (global id of the start hit).
+    """
+    pass
+
+
+class Oracle:
+    def __init__(self, n_sectors, n_rows, row_x, bz, params: Params | None = None, precision="float"):
+        self.n_sectors, self.n_rows = int(n_sectors), int(n_rows)
+        self._rx = np.ascontiguousarray(row_x, dtype=np.float32)
+        self.use_double = 1 if precision == "double" else 0
+        self._h = lib().oracle_create(self.n_sectors, self.n_rows, self._rx.ctypes.data, float(bz),
+                                      ctypes.byref(params) if params is not None else None, self.use_double)
+
+    def __del__(self):
+        try:
+            if self._h:
+                lib().oracle_destroy(self._h)
+                self._h = None
+        except Exception:
+            pass
+
+    def run(self, row_counts, y, z, brute_force=False, fetch=True) -> Result | None:
+        L = lib()
+        rc = np.ascontiguousarray(row_counts, dtype=np.int32).reshape(-1)
+        assert rc.size == self.n_sectors * self.n_rows
+        y = np.ascontiguousarray(y, dtype=np.float32)
+        z = np.ascontiguousarray(z, dtype=np.float32)
+        assert y.size == int(rc.sum()) == z.size
+        L.oracle_run(self._h, rc.ctypes.data, y.ctypes.data, z.ctypes.data, 1 if brute_force else 0)
+        return self.fetch() if fetch else None
+
+    def stage_seconds(self):
+        s = np.zeros(6)
+        lib().oracle_get_stage_seconds(self._h, s.ctypes.data)
+        return dict(zip(("grid", "neighbours", "clean", "start_hits", "construct", "select"), s.tolist()))
+
+    def fetch(self) -> Result:
+        L, h = lib(), self._h
+        r = Result()
+        n = L.oracle_n_clusters(h)
+        r.n_clusters = n
+        links = []
+        for which in range(4):
+            a = np.empty(n, dtype=np.int32)
+            L.oracle_get_links(h, which, a.ctypes.data)
+            links.append(a)
+        r.link_up, r.link_dn, r.link_up_clean, r.link_dn_clean = links
+        r.tie_s2 = np.empty(n, dtype=np.uint8)
+        L.oracle_get_tie_flags(h, r.tie_s2.ctypes.data)
+        ns = L.oracle_n_start_hits(h)
+        r.start_hits = np.empty(ns, dtype=np.int64)
+        L.oracle_get_start_hits(h, r.start_hits.ctypes.data)
+        m = L.oracle_n_tracklets(h)
+        r.tracklets = np.empty(m, dtype=TRACKLET_DTYPE)
+        r.row_hit = np.empty((m, self.n_rows), dtype=np.int32)
+        L.oracle_get_tracklets(h, r.tracklets.ctypes.data, r.row_hit.ctypes.data)
+        r.owner = np.empty(n, dtype=np.int64)
+        L.oracle_get_owners(h, r.owner.ctypes.data)
+        nt, nc = L.oracle_n_tracks(h), L.oracle_n_cluster_ids(h)
+        r.tracks = np.empty(nt, dtype=TRACK_DTYPE)
+        r.cluster_ids = np.empty(nc, dtype=np.int32)
+        L.oracle_get_tracks(h, r.tracks.ctypes.data, r.cluster_ids.ctypes.data)
+        return r
+
+
+def run_event(ev, params: Params | None = None, precision="float", brute_force=False) -> Result:
+    """Convenience: run the oracle on a datagen.Event-like object (duck-typed, no import of datagen)."""
+    o = Oracle(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz, params, precision)
+    return o.run(ev.row_counts, ev.y, ev.z, brute_force)
+
+
+def propagate(x, p, c, x2, cb, smax=0.95, precision="double"):
+    """One propagation step; returns (ok, x, p[5], c[15], J[5,5])."""
+    xa = np.array([x], dtype=np.float64)
+    pa = np.array(p, dtype=np.float64).copy()
+    ca = np.array(c, dtype=np.float64).copy()
+    J = np.zeros((5, 5))
+    ok = lib().oracle_propagate(1 if precision == "double" else 0, xa.ctypes.data, pa.ctypes.data, ca.ctypes.data,
+                                float(x2), float(cb), float(smax), J.ctypes.data)
+    return bool(ok), float(xa[0]), pa, ca, J
+
+
+def update(p, c, chi2, coord, m, e2, precision="double"):
+    """One scalar Kalman update; returns (p, c, chi2)."""
+    pa = np.array(p, dtype=np.float64).copy()
+    ca = np.array(c, dtype=np.float64).copy()
+    ch = np.array([chi2], dtype=np.float64)
+    lib().oracle_update(1 if precision == "double" else 0, pa.ctypes.data, ca.ctypes.data, ch.ctypes.data,
+                        int(coord), float(m), float(e2))
+    return pa, ca, float(ch[0])
