@@ -1,0 +1,163 @@
+/*
+ * tpctrk.h — C ABI of the B200-native Phase-I TPC sector tracker (libtpctrk.so).
+ *
+ * The calls follow the paper's statement of the problem (arxiv 1712.09430; PAPER.md = /root/reference/PAPER.md):
+ *   clusters (x,y,z) per TPC sector and pad row
+ *     -> Phase I, step 1: cellular-automaton seeding, one GPU thread per hit
+ *     -> Phase I, step 2: track following with a simplified Kalman filter, one thread per track
+ *        candidate, and selection of the best instance per track segment
+ *     -> tracklets with cluster lists and 5-parameter states plus covariances.
+ * The numerical readings (S0..S6, R-1..R-15) are listed in DESIGN.md.
+ *
+ * Conventions
+ *  - Plain C, no exceptions or aborts cross the ABI.  Every int-returning call returns TPC_OK (0) or a
+ *    negative tpc_error; tpc_strerror() names it.
+ *  - "device pointer" = CUDA device memory of the current device; "host pointer" = ordinary or pinned host
+ *    memory.  Where a call accepts either, the kind is detected with cudaPointerGetAttributes.
+ *  - All work is enqueued on the stream given to tpc_set_stream (default: the legacy default stream).
+ *    Calls are asynchronous unless stated otherwise.
+ *  - The library never allocates device memory for the hot path: the caller hands it one workspace
+ *    (tpc_set_workspace), e.g. a torch tensor, and keeps ownership.  Pinned host memory for result
+ *    download is library-owned.
+ *  - There is no CPU fallback: without a CUDA device every compute call returns TPC_E_CUDA.
+ */
+#ifndef TPCTRK_H
+#define TPCTRK_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tpc_tracker tpc_tracker; /* opaque, library-owned */
+
+typedef enum tpc_error {
+    TPC_OK = 0,
+    TPC_E_ARG = -1,      /* null pointer, sector/row/count out of range, unsupported geometry */
+    TPC_E_STATE = -2,    /* call out of order (no workspace, nothing loaded, nothing tracked yet) */
+    TPC_E_NOMEM = -3,    /* workspace too small for the loaded clusters; see tpc_workspace_bytes */
+    TPC_E_OVERFLOW = -4, /* tracklet-capacity estimate exceeded ("estimation was too small");
+                            tpc_stats.n_start_hits holds the required capacity; enlarge and re-run */
+    TPC_E_CUDA = -5      /* CUDA runtime error or no device; tpc_last_cuda_error() has the code */
+} tpc_error;
+
+/* Constants of the method (the paper gives none). */
+typedef struct tpc_params {
+    float err2_y, err2_z;           /* measurement variances [cm^2], uncorrelated          0.01 */
+    float nf_ty, nf_tz;             /* neighbour window slope limits |dy/dx|, |dz/dx|  1.0, 1.5 */
+    float nf_c;                     /* neighbour window padding [cm]                                      0.5 */
+    float nf_d2max;                 /* max squared 3-point collinearity residual [cm^2]                  0.25 */
+    float kf_css0, kf_ctt0, kf_ckk0;/* initial variances of sin(phi), dz/ds, q/pT                  1, 10, 100 */
+    float kf_smax;                  /* propagation fails for |sin(phi)| >= this            0.95 */
+    float road_nsig, road_max;      /* search road = min(road_max, nsig*sqrt(C+err2)) per coordinate   4, 2.0 */
+    int32_t max_gap;                /* a leg stops at the (max_gap+1)-th consecutive empty row              4 */
+    int32_t min_hits;               /* min hits of a kept tracklet and min owned hits of a track           10 */
+    int32_t seed_min_chain;         /* min link-chain length of a seed ("3 to about 10")        3 */
+    float max_tracklets_per_cluster;/* capacity estimate for tracklets                    0.125 */
+} tpc_params;
+
+typedef struct tpc_geometry {
+    int32_t n_sectors;        /* 36: s<18 side A (z>0), s>=18 side C (z<0); any value >= 1 works */
+    int32_t n_rows;           /* 159 pad rows; 3 <= n_rows <= 255 */
+    const float* row_x;       /* host pointer, n_rows ascending pad-row x [cm]; copied at create */
+    float sector_dphi;        /* informational: 20 deg in rad; all tracking is sector-local */
+    float z_max;              /* informational: drift length [cm] */
+    const tpc_params* params; /* host pointer or NULL = defaults */
+} tpc_geometry;
+
+/* One output track = one selected tracklet.  State is given at x (sector-local frame):
+ * p = (y, z, sin(phi), dz/ds, q/pT); c = lower triangle yy, zy,zz, sy,sz,ss, ty,tz,ts,tt, ky,kz,ks,kt,kk. */
+typedef struct tpc_track {
+    int32_t sector, n_clusters, first_row, last_row;
+    int32_t cluster_offset;   /* into cluster_ids; ids ascending in row, one per row */
+    float x;
+    float p[5];
+    float c[15];
+    float chi2;
+    int32_t n_fit;            /* number of hit updates in the final (inward) filter pass */
+} tpc_track;
+
+/* Counters and device times of the last tpc_track_sectors (valid after tpc_get_tracks / tpc_sync). */
+typedef struct tpc_stats {
+    int64_t n_clusters, n_links, n_start_hits, n_tracklets, n_tracklet_hits, n_tracks, n_track_clusters;
+    int64_t workspace_bytes_used, max_clusters, max_tracklets;
+    float kernel_us[8];       /* K1 sort+grid, K2 neighbours, K3/K4 clean+start, K5 construct, K6a weights,
+                                 K6b select+compact, [6] = K1..K6 total, [7] = unused */
+} tpc_stats;
+
+/* Record of tpc_debug_dump(TPC_DUMP_TRACKLETS). */
+typedef struct tpc_tracklet {
+    uint32_t start_gid;       /* event-global id of the start hit = canonical tracklet id */
+    int32_t sector, start_row, n_hits, first_row, last_row, n_fit;
+    float x, p[5], c[15], chi2;
+} tpc_tracklet;
+
+enum {
+    TPC_DUMP_LINKS = 1,       /* int32[4][N]: linkUp, linkDn after K2; linkUp, linkDn after K3.  Indexed by global id;
+                                 value = LOAD index of the linked hit inside row r+1 / r-1, -1 none */
+    TPC_DUMP_START_HITS = 2,  /* uint32[n_start_hits]: global ids, unordered */
+    TPC_DUMP_TRACKLETS = 3,   /* tpc_tracklet[n_start_hits] then int32[n_start_hits][n_rows] row->load index, -1 none */
+    TPC_DUMP_OWNERS = 4       /* uint32[N]: start_gid of the owning tracklet, 0xFFFFFFFF none */
+};
+
+/* Defaults of DESIGN.md "Constants". */
+void tpc_default_params(tpc_params* p);
+
+/* Create a tracker for a geometry and a constant field Bz [T].  g and its pointers are host
+ * memory, copied.  *out is owned by the library until tpc_tracker_destroy.  Does not touch the GPU. */
+int tpc_tracker_create(const tpc_geometry* g, float bz_tesla, tpc_tracker** out);
+void tpc_tracker_destroy(tpc_tracker* t);
+
+/* cuda_stream: a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = default stream. */
+int tpc_set_stream(tpc_tracker* t, void* cuda_stream);
+
+/* Device bytes needed for events of up to max_clusters clusters (internal buffers). */
+size_t tpc_workspace_bytes(const tpc_tracker* t, int64_t max_clusters);
+/* dev_ptr: device pointer, 256-byte aligned, caller-owned, must outlive its use.  Capacity is derived from bytes. */
+int tpc_set_workspace(tpc_tracker* t, void* dev_ptr, size_t bytes);
+
+/* Forget all loaded clusters. */
+int tpc_reset_event(tpc_tracker* t);
+
+/* Load the n clusters of one (sector,row).  x, y, z: n floats each, all host or all device pointers; copied
+ * (device: enqueued on the stream; host: staged in pinned memory, uploaded by tpc_track_sectors).  x may be NULL and
+ * is not used: the tracker takes the pad-row x (R-13).  Index i in this call is the cluster's load index;
+ * its event-global id is rowBase(sector,row)+i with rowBase the exclusive prefix sum of the loaded counts in
+ * ascending (sector,row) order.  Loading a (sector,row) again replaces it.  Non-finite coordinates give undefined
+ * tracks but never a crash or hang. */
+int tpc_load_clusters(tpc_tracker* t, int sector, int row, int n, const float* x, const float* y, const float* z);
+
+/* Load a whole event at once: row_counts[n_sectors*n_rows] on the host; y, z concatenated in ascending (sector,row)
+ * order, both host or both device pointers.  Replaces everything loaded before. */
+int tpc_load_event(tpc_tracker* t, const int32_t* row_counts, const float* y, const float* z);
+
+/* Run K1..K6 (sort+grid, neighbours finder, cleaner+start hits, tracklet constructor, selector+compaction) on the
+ * stream.  Asynchronous.  May be called repeatedly on the same loaded event. */
+int tpc_track_sectors(tpc_tracker* t);
+
+/* Synchronise, download the result into library-owned pinned memory (valid until the next track/reset/destroy).
+ * tracks[i].cluster_offset indexes cluster_ids (event-global ids).  Track order is unspecified.
+ * Returns TPC_E_OVERFLOW if the tracklet capacity was exceeded (results then cover the first max_tracklets seeds). */
+int tpc_get_tracks(tpc_tracker* t, const tpc_track** tracks, int32_t* n_tracks,
+                   const uint32_t** cluster_ids, int64_t* n_cluster_ids);
+
+/* Synchronise the stream and fetch counters + per-kernel device times only (no track download). */
+int tpc_sync(tpc_tracker* t);
+int tpc_get_stats(tpc_tracker* t, tpc_stats* out);
+
+/* Stage parity hooks (tests): copy one stage's buffers, converted to canonical (load-index) form, to host_dst.
+ * Synchronous; allocates temporary device memory.  bytes must equal tpc_debug_dump_bytes(t, stage). */
+size_t tpc_debug_dump_bytes(tpc_tracker* t, int stage);
+int tpc_debug_dump(tpc_tracker* t, int stage, void* host_dst, size_t bytes);
+
+const char* tpc_strerror(int code);
+int tpc_last_cuda_error(const tpc_tracker* t);
+/* Number of kernel launches one tpc_track_sectors enqueues (for bench.py's gpu_launches). */
+int tpc_launches_per_track(const tpc_tracker* t);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TPCTRK_H */

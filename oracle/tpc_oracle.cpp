@@ -62,22 +62,26 @@ template <class T> bool propagate(State<T> &st, T x2, T CB, T smax, T (*Jout)[5]
     const T c2 = std::sqrt(T(1) - s2 * s2);
     const T cc = c + c2;
     const T ss = s + s2;
-    const T tg = ss / cc;                       /* tan of the mean direction */
+    const T rcc = T(1) / cc;
+    const T tg = ss * rcc;                      /* tan of the mean direction */
+    const T q = std::sqrt(T(1) + tg * tg);
     const T dy = dx * tg;
-    const T l = dx * std::sqrt(T(1) + tg * tg); /* signed chord */
+    const T l = dx * q;                         /* signed chord */
     const T a = (T(0.5) * kap) * l;
     const T a2 = a * a;
     const T c16 = T(1) / T(6), c340 = T(3) / T(40);
     const T dS = l * (T(1) + a2 * (c16 + a2 * c340)); /* arc = chord * asin(a)/a, series */
-    const T icc = cc * cc;
-    const T d1 = ((ss * s) / c + cc) / icc;     /* d tg / d s  */
-    const T d2 = ((ss * s2) / c2 + cc) / icc;   /* d tg / d s2 */
+    const T rc = T(1) / c, rc2 = T(1) / c2;
+    const T rcc2 = rcc * rcc;
+    const T d1 = ((ss * s) * rc + cc) * rcc2;   /* d tg / d s  */
+    const T d2 = ((ss * s2) * rc2 + cc) * rcc2; /* d tg / d s2 */
     T J[5][5];
     for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) J[i][j] = (i == j) ? T(1) : T(0);
     J[0][2] = dx * (d1 + d2);
     J[0][4] = ((dx * d2) * CB) * dx;
     J[2][4] = CB * dx;
-    const T sm = dy / l;                        /* d l / d tg = dx*sm, so d l / d s = sm*J[y][s] */
+    const T rq = T(1) / q;
+    const T sm = tg * rq;                       /* = dy/l; d l / d tg = dx*sm, so d l / d s = sm*J[y][s] */
     const T tsm = t * sm;
     const T h = T(1) + a2 * (T(0.5) + a2 * T(0.375));   /* d dS / d l at fixed curvature */
     const T gp = c16 + a2 * (T(3) / T(20));             /* d (dS/l) / d a2 */
@@ -113,8 +117,9 @@ template <class T> bool propagate(State<T> &st, T x2, T CB, T smax, T (*Jout)[5]
 template <class T> void update1(State<T> &st, int i, T m, T e2) {
     const T r = m - st.p[i];
     const T S = st.C[i][i] + e2;
+    const T w = T(1) / S;
     T K[5], row[5];
-    for (int a = 0; a < 5; a++) { K[a] = st.C[a][i] / S; row[a] = st.C[i][a]; }
+    for (int a = 0; a < 5; a++) { K[a] = st.C[a][i] * w; row[a] = st.C[i][a]; }
     for (int a = 0; a < 5; a++) st.p[a] = st.p[a] + K[a] * r;
     for (int a = 0; a < 5; a++)
         for (int b = 0; b <= a; b++) {
@@ -122,7 +127,7 @@ template <class T> void update1(State<T> &st, int i, T m, T e2) {
             st.C[a][b] = v;
             st.C[b][a] = v;
         }
-    st.chi2 = st.chi2 + (r * r) / S;
+    st.chi2 = st.chi2 + (r * r) * w;
 }
 
 /* A hit = two sequential scalar updates, y first, then z (uncorrelated errors). */

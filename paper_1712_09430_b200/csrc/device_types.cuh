@@ -1,0 +1,74 @@
+// Device-side data layout of the tracker.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "tpctrk.h"
+
+namespace tpc {
+
+constexpr int kMaxRows = 255;          // n_rows limit: nHits must fit the 8-bit field of the ownership key
+constexpr int kRowPad = 4;             // a row's sorted hits start at a multiple of 4 hits (32 B sector, 16 B TMA)
+constexpr int kMaxBinsPerRow = 8192;   // K1 histogram lives in shared memory (32 KB)
+constexpr float kGridMargin = 1e-3f;   // [cm] slack of every bin-range query; the exact window test follows
+
+// One (sector,row).  Host fills the first 8 words when an event is finalised; K1 fills the grid.
+struct __align__(16) RowInfo {
+    int32_t hitOff;    // offset of the row's sorted hits in hits[]/orig[]/links/weight (multiple of kRowPad)
+    int32_t n;         // clusters in the row
+    int32_t inOff;     // offset of the row's clusters in the staging arrays, as loaded
+    int32_t binOff;    // offset of the row's binStart[nBins+1]
+    uint32_t gidBase;  // event-global id of load index 0 (canonical ids)
+    int32_t maxBins;   // capacity reserved for this row's bins
+    int32_t nY, nZ;    // grid dimensions (K1)
+    float y0, z0;      // grid origin (K1)
+    float invY, invZ;  // 1 / bin size (K1)
+};
+static_assert(sizeof(RowInfo) == 48, "RowInfo layout");
+
+// Per-tracklet record written by K5 (128 B, float4-aligned).
+struct __align__(16) TrackletRec {
+    uint32_t startGid;
+    int32_t sector, startRow, nHits, firstRow, lastRow, nFit, xRow;
+    float p[5];
+    float c[15];
+    float chi2;
+    float pad[3];
+};
+static_assert(sizeof(TrackletRec) == 128, "TrackletRec layout");
+
+struct DevParams {
+    tpc_params P;
+    float CB;          // curvature per unit q/pT: kappa = p[4]*CB  [1/cm per c/GeV]
+    int32_t nSec, nRows;
+};
+
+enum Counter { kNStart = 0, kQueue = 1, kNTracks = 2, kNTrackClusters = 3, kNKept = 4, kHitsTotal = 5, kNLinks = 6, kNCounters = 16 };
+
+// All device pointers of one tracker; passed by value to the kernels.
+struct DevPtrs {
+    const float* inY;
+    const float* inZ;
+    RowInfo* rows;
+    const float* rowX;
+    float2* hits;          // sorted (y,z) pairs
+    uint32_t* orig;        // sorted position -> load index
+    uint32_t* binStart;
+    int32_t* linkUp;       // raw links, index = sorted position in the adjacent row
+    int32_t* linkDn;
+    int32_t* linkUpC;      // cleaned links
+    int32_t* linkDnC;
+    uint32_t* weight;      // ownership key per hit
+    int2* starts;          // (rowId, sorted position)
+    TrackletRec* recs;
+    int32_t* rowHit;       // [maxTracklets][rhStride], sorted position of the tracklet's hit in each row, -1 none
+    tpc_track* tracks;
+    uint32_t* clusterIds;
+    uint32_t* counters;
+    uint32_t* sectorGidBase;
+    int32_t nRowsTotal;
+    int32_t maxTracklets;
+    int32_t rhStride;      // n_rows rounded up to a multiple of 32
+};
+
+}  // namespace tpc

@@ -1,0 +1,272 @@
+// K1 cluster sort + row grid, K2 neighbours finder, K3/K4 neighbours cleaner + start-hit finder.
+// Phase I step 1, "seeding ... heuristics in a cellular automaton", one GPU thread per hit
+// (PAPER.md:33,66); readings S1..S4 of DESIGN.md.  Compiled with -fmad=false: every decision value is the
+// IEEE fp32 result of the written expression (R-12).
+#pragma once
+#include "device_types.cuh"
+
+namespace tpc {
+
+// Bin index of coordinate v: monotone non-decreasing in v, total (NaN -> 0), used for hits AND queries.
+__device__ __forceinline__ int bin_of(float v, float v0, float inv, int n) {
+    float f = (v - v0) * inv;
+    f = fminf(fmaxf(f, 0.0f), (float)(n - 1));
+    return (int)f;
+}
+
+// ------------------------------------------------------------------------------------------ K1
+// One block per (sector,row): bounding box -> grid -> histogram in shared memory -> scan -> scatter.
+// Input: SoA y[], z[] as loaded (coalesced reads).  Output: sorted float2 (y,z), orig[], binStart[], grid.
+constexpr int kK1Threads = 256;
+
+__global__ void __launch_bounds__(kK1Threads) k1_sort_grid(DevPtrs d) {
+    const int rowId = blockIdx.x;
+    const int tid = threadIdx.x;
+    if (rowId == 0 && tid < kNCounters) d.counters[tid] = 0u;
+    RowInfo R = d.rows[rowId];
+    const int n = R.n;
+    if (n == 0) return;
+    extern __shared__ uint32_t sh[];            // [maxBins + 1] histogram / cursors
+    __shared__ float redA[4][kK1Threads / 32];
+    __shared__ uint32_t warpSum[kK1Threads / 32];
+    __shared__ int sNY, sNZ;
+    __shared__ float sY0, sZ0, sInvY, sInvZ;
+    const float* __restrict__ y = d.inY + R.inOff;
+    const float* __restrict__ z = d.inZ + R.inOff;
+
+    // 1. bounding box
+    float ymin = 3.0e38f, ymax = -3.0e38f, zmin = 3.0e38f, zmax = -3.0e38f;
+    for (int i = tid; i < n; i += kK1Threads) {
+        const float a = y[i], b = z[i];
+        ymin = fminf(ymin, a); ymax = fmaxf(ymax, a);
+        zmin = fminf(zmin, b); zmax = fmaxf(zmax, b);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        ymin = fminf(ymin, __shfl_xor_sync(0xffffffffu, ymin, o));
+        ymax = fmaxf(ymax, __shfl_xor_sync(0xffffffffu, ymax, o));
+        zmin = fminf(zmin, __shfl_xor_sync(0xffffffffu, zmin, o));
+        zmax = fmaxf(zmax, __shfl_xor_sync(0xffffffffu, zmax, o));
+    }
+    if ((tid & 31) == 0) { redA[0][tid >> 5] = ymin; redA[1][tid >> 5] = ymax; redA[2][tid >> 5] = zmin; redA[3][tid >> 5] = zmax; }
+    __syncthreads();
+    if (tid == 0) {
+        for (int w = 1; w < kK1Threads / 32; w++) {
+            ymin = fminf(ymin, redA[0][w]); ymax = fmaxf(ymax, redA[1][w]);
+            zmin = fminf(zmin, redA[2][w]); zmax = fmaxf(zmax, redA[3][w]);
+        }
+        // non-finite input must not blow the grid up
+        ymin = fminf(fmaxf(ymin, -1.0e4f), 1.0e4f); ymax = fminf(fmaxf(ymax, -1.0e4f), 1.0e4f);
+        zmin = fminf(fmaxf(zmin, -1.0e4f), 1.0e4f); zmax = fminf(fmaxf(zmax, -1.0e4f), 1.0e4f);
+        const float spanY = fmaxf(ymax - ymin, 1.0e-2f), spanZ = fmaxf(zmax - zmin, 1.0e-2f);
+        // about one hit per bin, bins twice as long in z as in y (a query costs per z-bin-row), >= 0.5 cm
+        const int target = max(1, min(R.maxBins, n));
+        float ey = sqrtf(spanY * spanZ / (2.0f * (float)target));
+        ey = fmaxf(ey, 0.5f);
+        int nY = max(1, min(target, (int)(spanY / ey)));
+        int nZ = max(1, min(target / nY, (int)(spanZ / (2.0f * ey))));
+        sNY = nY; sNZ = nZ; sY0 = ymin; sZ0 = zmin;
+        sInvY = (float)nY / spanY; sInvZ = (float)nZ / spanZ;
+        R.nY = nY; R.nZ = nZ; R.y0 = ymin; R.z0 = zmin; R.invY = sInvY; R.invZ = sInvZ;
+        d.rows[rowId] = R;
+    }
+    __syncthreads();
+    const int nY = sNY, nZ = sNZ, nBins = nY * nZ;
+    const float y0 = sY0, z0 = sZ0, invY = sInvY, invZ = sInvZ;
+
+    // 2. histogram
+    for (int b = tid; b <= nBins; b += kK1Threads) sh[b] = 0u;
+    __syncthreads();
+    for (int i = tid; i < n; i += kK1Threads) {
+        const int b = bin_of(z[i], z0, invZ, nZ) * nY + bin_of(y[i], y0, invY, nY);
+        atomicAdd(&sh[b], 1u);
+    }
+    __syncthreads();
+
+    // 3. exclusive scan of sh[0..nBins] (chunk per thread, warp shuffles across chunks)
+    const int chunk = (nBins + 1 + kK1Threads - 1) / kK1Threads;
+    const int b0 = min(tid * chunk, nBins + 1), b1 = min(b0 + chunk, nBins + 1);
+    uint32_t local = 0;
+    for (int b = b0; b < b1; b++) local += sh[b];
+    uint32_t incl = local;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
+        if ((tid & 31) >= o) incl += v;
+    }
+    if ((tid & 31) == 31) warpSum[tid >> 5] = incl;
+    __syncthreads();
+    uint32_t base = incl - local;
+    for (int w = 0; w < (tid >> 5); w++) base += warpSum[w];
+    uint32_t* __restrict__ bs = d.binStart + R.binOff;
+    for (int b = b0; b < b1; b++) {
+        const uint32_t c = sh[b];
+        sh[b] = base;          // becomes the scatter cursor
+        bs[b] = base;
+        base += c;
+    }
+    __syncthreads();
+
+    // 4. scatter (order inside a bin is arbitrary: no result depends on it, tie-breaks use orig[])
+    float2* __restrict__ hs = d.hits + R.hitOff;
+    uint32_t* __restrict__ og = d.orig + R.hitOff;
+    uint32_t* __restrict__ wt = d.weight + R.hitOff;
+    for (int i = tid; i < n; i += kK1Threads) {
+        const float a = y[i], c = z[i];
+        const int b = bin_of(c, z0, invZ, nZ) * nY + bin_of(a, y0, invY, nY);
+        const uint32_t pos = atomicAdd(&sh[b], 1u);
+        hs[pos] = make_float2(a, c);
+        og[pos] = (uint32_t)i;
+        wt[i] = 0u;
+    }
+}
+
+// Enumerate every hit of row R whose bin overlaps [yc-wy, yc+wy] x [zc-wz, zc+wz] (a superset of the window).
+template <class F>
+__device__ __forceinline__ void for_window(const RowInfo& R, const float2* __restrict__ hits,
+                                           const uint32_t* __restrict__ binStart, float yc, float zc, float wy,
+                                           float wz, F&& f) {
+    const int by0 = bin_of(yc - wy - kGridMargin, R.y0, R.invY, R.nY);
+    const int by1 = bin_of(yc + wy + kGridMargin, R.y0, R.invY, R.nY);
+    const int bz0 = bin_of(zc - wz - kGridMargin, R.z0, R.invZ, R.nZ);
+    const int bz1 = bin_of(zc + wz + kGridMargin, R.z0, R.invZ, R.nZ);
+    const uint32_t* __restrict__ bs = binStart + R.binOff;
+    const float2* __restrict__ hs = hits + R.hitOff;
+    for (int bz = bz0; bz <= bz1; bz++) {
+        const int k0 = (int)bs[bz * R.nY + by0], k1 = (int)bs[bz * R.nY + by1 + 1];
+        for (int k = k0; k < k1; k++) f(k, hs[k]);
+    }
+}
+
+// ------------------------------------------------------------------------------------------ K2
+// Neighbours finder (S2): for each hit the best (up,down) pair in rows r+1/r-1 by 3-point collinearity.
+constexpr int kK2Threads = 128;
+constexpr int kK2Cap = 16;   // down-candidates cached per thread; beyond that a nested rescan (slow, exact)
+
+__global__ void __launch_bounds__(kK2Threads) k2_neighbours(DevPtrs d, DevParams dp) {
+    const int rowId = blockIdx.x;
+    const int r = rowId % dp.nRows;
+    const RowInfo R = d.rows[rowId];
+    if (R.n == 0) return;
+    int32_t* __restrict__ up = d.linkUp + R.hitOff;
+    int32_t* __restrict__ dn = d.linkDn + R.hitOff;
+    bool active = (r >= 1 && r <= dp.nRows - 2);
+    RowInfo Ru, Rd;
+    if (active) {
+        Ru = d.rows[rowId + 1]; Rd = d.rows[rowId - 1];
+        active = Ru.n > 0 && Rd.n > 0;
+    }
+    if (!active) {
+        for (int i = threadIdx.x; i < R.n; i += kK2Threads) { up[i] = -1; dn[i] = -1; }
+        return;
+    }
+    const float xr = d.rowX[r];
+    const float dxu = d.rowX[r + 1] - xr;
+    const float dxd = d.rowX[r - 1] - xr;
+    const float wu = -dxd / (dxu - dxd), wd = dxu / (dxu - dxd);
+    const float wyU = dp.P.nf_ty * dxu + dp.P.nf_c, wzU = dp.P.nf_tz * dxu + dp.P.nf_c;
+    const float wyD = dp.P.nf_ty * (-dxd) + dp.P.nf_c, wzD = dp.P.nf_tz * (-dxd) + dp.P.nf_c;
+    const uint32_t* __restrict__ origU = d.orig + Ru.hitOff;
+    const uint32_t* __restrict__ origD = d.orig + Rd.hitOff;
+
+    for (int i = threadIdx.x; i < R.n; i += kK2Threads) {
+        const float2 h = d.hits[R.hitOff + i];
+        float cy[kK2Cap], cz[kK2Cap];
+        int ck[kK2Cap];
+        int nd = 0;
+        for_window(Rd, d.hits, d.binStart, h.x, h.y, wyD, wzD, [&](int k, float2 c) {
+            if (fabsf(c.x - h.x) <= wyD && fabsf(c.y - h.y) <= wzD) {
+                if (nd < kK2Cap) { cy[nd] = wd * c.x; cz[nd] = wd * c.y; ck[nd] = k; }
+                nd++;
+            }
+        });
+        int bestU = -1, bestD = -1;
+        float best = 0.0f;
+        auto consider = [&](int ku, int kd, float d2) {
+            bool better = bestU < 0 || d2 < best;
+            if (!better && d2 == best) {   // exact tie: smaller load index of u, then of d
+                const uint32_t ou = origU[ku], ob = origU[bestU];
+                better = ou < ob || (ou == ob && origD[kd] < origD[bestD]);
+            }
+            if (better) { best = d2; bestU = ku; bestD = kd; }
+        };
+        if (nd > 0) {
+            for_window(Ru, d.hits, d.binStart, h.x, h.y, wyU, wzU, [&](int ku, float2 c) {
+                if (!(fabsf(c.x - h.x) <= wyU && fabsf(c.y - h.y) <= wzU)) return;
+                const float py = wu * c.x, pz = wu * c.y;
+                if (nd <= kK2Cap) {
+                    for (int j = 0; j < nd; j++) {
+                        const float ey = h.x - (py + cy[j]), ez = h.y - (pz + cz[j]);
+                        consider(ku, ck[j], ey * ey + ez * ez);
+                    }
+                } else {
+                    for_window(Rd, d.hits, d.binStart, h.x, h.y, wyD, wzD, [&](int kd, float2 e) {
+                        if (!(fabsf(e.x - h.x) <= wyD && fabsf(e.y - h.y) <= wzD)) return;
+                        const float ey = h.x - (py + wd * e.x), ez = h.y - (pz + wd * e.y);
+                        consider(ku, kd, ey * ey + ez * ez);
+                    });
+                }
+            });
+        }
+        const bool ok = bestU >= 0 && best <= dp.P.nf_d2max;
+        up[i] = ok ? bestU : -1;
+        dn[i] = ok ? bestD : -1;
+    }
+}
+
+// ------------------------------------------------------------------------------------------ K3 + K4
+// Cleaner (S3): keep reciprocal links only.  Start hits (S4): no down-link, chain of >= seed_min_chain hits.
+// The chain test re-derives the cleaned up-links of the next rows from the raw links (same predicate), so one
+// kernel does both; the start list is appended with one atomic per warp (ballot + prefix).
+constexpr int kK3Threads = 128;
+
+__device__ __forceinline__ int clean_up_link(const DevPtrs& d, const RowInfo& R, const RowInfo& Rup, int i) {
+    const int u = d.linkUp[R.hitOff + i];
+    return (u >= 0 && d.linkDn[Rup.hitOff + u] == i) ? u : -1;
+}
+
+__global__ void __launch_bounds__(kK3Threads) k3_clean_start(DevPtrs d, DevParams dp) {
+    const int rowId = blockIdx.x;
+    const int r = rowId % dp.nRows;
+    const RowInfo R = d.rows[rowId];
+    if (R.n == 0) return;
+    const bool hasUp = r + 1 < dp.nRows, hasDn = r >= 1;
+    RowInfo Ru = R, Rd = R;
+    if (hasUp) Ru = d.rows[rowId + 1];
+    if (hasDn) Rd = d.rows[rowId - 1];
+    const unsigned lane = threadIdx.x & 31u;
+    unsigned nLinks = 0;
+    for (int base = 0; base < R.n; base += kK3Threads) {
+        const int i = base + threadIdx.x;
+        bool isStart = false;
+        if (i < R.n) {
+            const int u = d.linkUp[R.hitOff + i], dnl = d.linkDn[R.hitOff + i];
+            const int uc = (u >= 0 && d.linkDn[Ru.hitOff + u] == i) ? u : -1;
+            const int dc = (dnl >= 0 && d.linkUp[Rd.hitOff + dnl] == i) ? dnl : -1;
+            d.linkUpC[R.hitOff + i] = uc;
+            d.linkDnC[R.hitOff + i] = dc;
+            nLinks += uc >= 0;
+            if (dc < 0 && uc >= 0) {
+                int len = 2, cur = uc, row = rowId + 1;
+                while (len < dp.P.seed_min_chain && (row % dp.nRows) + 1 < dp.nRows) {
+                    const int nx = clean_up_link(d, d.rows[row], d.rows[row + 1], cur);
+                    if (nx < 0) break;
+                    cur = nx; row++; len++;
+                }
+                isStart = len >= dp.P.seed_min_chain;
+            }
+        }
+        const unsigned m = __ballot_sync(0xffffffffu, isStart);
+        if (m) {
+            unsigned pos = 0;
+            if (lane == 0) pos = atomicAdd(&d.counters[kNStart], (unsigned)__popc(m));
+            pos = __shfl_sync(0xffffffffu, pos, 0) + __popc(m & ((1u << lane) - 1u));
+            if (isStart && pos < (unsigned)d.maxTracklets) d.starts[pos] = make_int2(rowId, i);
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) nLinks += __shfl_xor_sync(0xffffffffu, nLinks, o);
+    if (lane == 0 && nLinks) atomicAdd(&d.counters[kNLinks], nLinks);
+}
+
+}  // namespace tpc

@@ -1,0 +1,556 @@
+// libtpctrk.so — C ABI (include/tpctrk.h) and host logic of the B200 Phase-I TPC sector tracker.
+// Every step of the hot path runs in the kernels of kernels_ca.cuh / kernels_kf.cuh; this file only lays out
+// the workspace, stages input, launches K1..K6 on the caller's stream and downloads the compacted result.
+// There is no CPU fallback: without a device the compute calls return TPC_E_CUDA.
+#include <algorithm>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "device_types.cuh"
+#include "kernels_ca.cuh"
+#include "kernels_kf.cuh"
+
+using namespace tpc;
+
+namespace {
+
+constexpr size_t kAlign = 256;
+inline size_t align_up(size_t v, size_t a = kAlign) { return (v + a - 1) / a * a; }
+
+struct Layout {   // byte offsets into the workspace
+    size_t inY, inZ, rows, rowX, hits, orig, binStart, linkUp, linkDn, linkUpC, linkDnC, weight, starts, recs, rowHit,
+        tracks, clusterIds, counters, sectorGidBase, total;
+    int64_t hitCap, binCap, maxTracklets;
+};
+
+}  // namespace
+
+struct tpc_tracker {
+    int nSec = 0, nRows = 0, nRowsTotal = 0, rhStride = 0;
+    std::vector<float> rowX;
+    tpc_params P{};
+    float bz = 0.f, CB = 0.f;
+    cudaStream_t stream = nullptr;
+    int lastCuda = 0;
+
+    // workspace
+    char* ws = nullptr;
+    size_t wsBytes = 0;
+    int64_t maxClusters = 0;
+    Layout L{};
+    DevPtrs dev{};
+
+    // loaded event (host bookkeeping)
+    std::vector<int32_t> rowN, rowIn;       // per (sector,row): count, staging offset
+    int64_t cursor = 0;                     // next free staging slot
+    int64_t nClusters = 0;
+    bool finalized = false, tracked = false, fetched = false;
+    float* hostY = nullptr; float* hostZ = nullptr; int64_t hostCap = 0;   // pinned mirror for host-pointer loads
+    int64_t dirtyLo = 0, dirtyHi = 0;
+    RowInfo* hostRows = nullptr;            // pinned
+    uint32_t* hostSectorBase = nullptr;     // pinned
+    uint32_t* hostCounters = nullptr;       // pinned
+    int maxBinsLaunch = 1;
+
+    // results (pinned)
+    tpc_track* outTracks = nullptr; int64_t outTracksCap = 0;
+    uint32_t* outIds = nullptr; int64_t outIdsCap = 0;
+    uint32_t counters[kNCounters] = {0};
+    cudaEvent_t ev[8] = {nullptr};
+    bool haveEvents = false;
+    float kernelUs[8] = {0};
+    int k5Blocks = 0, k6Blocks = 0;
+};
+
+namespace {
+
+#define CUDA_TRY(t, expr)                                             \
+    do {                                                              \
+        cudaError_t _e = (expr);                                      \
+        if (_e != cudaSuccess) { (t)->lastCuda = (int)_e; return TPC_E_CUDA; } \
+    } while (0)
+
+Layout make_layout(const tpc_tracker* t, int64_t maxClusters) {
+    Layout L{};
+    const int64_t NR = t->nRowsTotal;
+    L.hitCap = maxClusters + (int64_t)kRowPad * NR + 16;
+    L.binCap = maxClusters + 2 * NR + 16;
+    L.maxTracklets = (int64_t)((double)maxClusters * (double)t->P.max_tracklets_per_cluster) + 4096;
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t r = o; o = align_up(o + bytes); return r; };
+    L.inY = take(sizeof(float) * (maxClusters + 16));
+    L.inZ = take(sizeof(float) * (maxClusters + 16));
+    L.rows = take(sizeof(RowInfo) * (NR + 2));
+    L.rowX = take(sizeof(float) * (t->nRows + 1));
+    L.hits = take(sizeof(float2) * L.hitCap);
+    L.orig = take(sizeof(uint32_t) * L.hitCap);
+    L.binStart = take(sizeof(uint32_t) * L.binCap);
+    L.linkUp = take(sizeof(int32_t) * L.hitCap);
+    L.linkDn = take(sizeof(int32_t) * L.hitCap);
+    L.linkUpC = take(sizeof(int32_t) * L.hitCap);
+    L.linkDnC = take(sizeof(int32_t) * L.hitCap);
+    L.weight = take(sizeof(uint32_t) * L.hitCap);
+    L.starts = take(sizeof(int2) * L.maxTracklets);
+    L.recs = take(sizeof(TrackletRec) * L.maxTracklets);
+    L.rowHit = take(sizeof(int32_t) * L.maxTracklets * t->rhStride);
+    L.tracks = take(sizeof(tpc_track) * L.maxTracklets);
+    L.clusterIds = take(sizeof(uint32_t) * (maxClusters + 16));
+    L.counters = take(sizeof(uint32_t) * kNCounters);
+    L.sectorGidBase = take(sizeof(uint32_t) * (t->nSec + 1));
+    L.total = o;
+    return L;
+}
+
+void bind_pointers(tpc_tracker* t) {
+    char* w = t->ws;
+    const Layout& L = t->L;
+    DevPtrs& d = t->dev;
+    d.inY = (const float*)(w + L.inY); d.inZ = (const float*)(w + L.inZ);
+    d.rows = (RowInfo*)(w + L.rows); d.rowX = (const float*)(w + L.rowX);
+    d.hits = (float2*)(w + L.hits); d.orig = (uint32_t*)(w + L.orig); d.binStart = (uint32_t*)(w + L.binStart);
+    d.linkUp = (int32_t*)(w + L.linkUp); d.linkDn = (int32_t*)(w + L.linkDn);
+    d.linkUpC = (int32_t*)(w + L.linkUpC); d.linkDnC = (int32_t*)(w + L.linkDnC);
+    d.weight = (uint32_t*)(w + L.weight); d.starts = (int2*)(w + L.starts);
+    d.recs = (TrackletRec*)(w + L.recs); d.rowHit = (int32_t*)(w + L.rowHit);
+    d.tracks = (tpc_track*)(w + L.tracks); d.clusterIds = (uint32_t*)(w + L.clusterIds);
+    d.counters = (uint32_t*)(w + L.counters); d.sectorGidBase = (uint32_t*)(w + L.sectorGidBase);
+    d.nRowsTotal = t->nRowsTotal; d.maxTracklets = (int32_t)std::min<int64_t>(L.maxTracklets, 0x7fffffff);
+    d.rhStride = t->rhStride;
+}
+
+bool is_device_pointer(const void* p) {
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+int ensure_host_stage(tpc_tracker* t, int64_t need) {
+    if (need <= t->hostCap) return TPC_OK;
+    int64_t cap = std::max<int64_t>(need, t->hostCap * 2);
+    cap = std::min<int64_t>(std::max<int64_t>(cap, 1 << 16), std::max<int64_t>(t->maxClusters, need));
+    float *ny = nullptr, *nz = nullptr;
+    CUDA_TRY(t, cudaMallocHost(&ny, sizeof(float) * cap));
+    CUDA_TRY(t, cudaMallocHost(&nz, sizeof(float) * cap));
+    if (t->hostY) {
+        // pending async uploads read the old buffers: drain them first
+        CUDA_TRY(t, cudaStreamSynchronize(t->stream));
+        std::memcpy(ny, t->hostY, sizeof(float) * t->hostCap);
+        std::memcpy(nz, t->hostZ, sizeof(float) * t->hostCap);
+        cudaFreeHost(t->hostY); cudaFreeHost(t->hostZ);
+    }
+    t->hostY = ny; t->hostZ = nz; t->hostCap = cap;
+    return TPC_OK;
+}
+
+// Host "initialisation" of an event (PAPER.md:66 host pre-processing, reduced to a prefix sum over row counts):
+// canonical id bases, padded row offsets, bin capacities; uploads the row table and any host-staged clusters.
+int finalize_event(tpc_tracker* t) {
+    if (t->finalized) return TPC_OK;
+    const int NR = t->nRowsTotal;
+    if (!t->hostRows) {
+        CUDA_TRY(t, cudaMallocHost(&t->hostRows, sizeof(RowInfo) * (NR + 2)));
+        CUDA_TRY(t, cudaMallocHost(&t->hostSectorBase, sizeof(uint32_t) * (t->nSec + 1)));
+        CUDA_TRY(t, cudaMallocHost(&t->hostCounters, sizeof(uint32_t) * kNCounters));
+    } else {
+        CUDA_TRY(t, cudaStreamSynchronize(t->stream));   // a previous async upload may still read hostRows
+    }
+    int64_t gid = 0, hitOff = 0, binOff = 0;
+    int maxBins = 1;
+    for (int i = 0; i < NR; i++) {
+        RowInfo& R = t->hostRows[i];
+        std::memset(&R, 0, sizeof(R));
+        if (i % t->nRows == 0) {
+            t->hostSectorBase[i / t->nRows] = (uint32_t)gid;
+        }
+        const int n = t->rowN[i];
+        R.hitOff = (int32_t)hitOff; R.n = n; R.inOff = t->rowIn[i]; R.binOff = (int32_t)binOff;
+        R.gidBase = (uint32_t)gid;
+        R.maxBins = std::max(1, std::min(n, kMaxBinsPerRow));
+        R.nY = R.nZ = 1; R.invY = R.invZ = 1.f;
+        maxBins = std::max(maxBins, R.maxBins);
+        gid += n;
+        hitOff += (n + kRowPad - 1) / kRowPad * kRowPad;
+        binOff += R.maxBins + 1;
+    }
+    t->hostSectorBase[t->nSec] = (uint32_t)gid;
+    for (int s = 0; s < t->nSec; s++)
+        if ((int64_t)t->hostSectorBase[s + 1] - (int64_t)t->hostSectorBase[s] > 0x00FFFFFF) return TPC_E_ARG;  // key field
+    t->nClusters = gid;
+    t->maxBinsLaunch = maxBins;
+    if (gid > t->maxClusters || hitOff > t->L.hitCap || binOff > t->L.binCap) return TPC_E_NOMEM;
+    CUDA_TRY(t, cudaMemcpyAsync(t->dev.rows, t->hostRows, sizeof(RowInfo) * NR, cudaMemcpyHostToDevice, t->stream));
+    CUDA_TRY(t, cudaMemcpyAsync(t->dev.sectorGidBase, t->hostSectorBase, sizeof(uint32_t) * (t->nSec + 1),
+                                cudaMemcpyHostToDevice, t->stream));
+    if (t->dirtyHi > t->dirtyLo) {
+        const int64_t lo = t->dirtyLo, cnt = t->dirtyHi - t->dirtyLo;
+        CUDA_TRY(t, cudaMemcpyAsync((float*)t->dev.inY + lo, t->hostY + lo, sizeof(float) * cnt, cudaMemcpyHostToDevice, t->stream));
+        CUDA_TRY(t, cudaMemcpyAsync((float*)t->dev.inZ + lo, t->hostZ + lo, sizeof(float) * cnt, cudaMemcpyHostToDevice, t->stream));
+        t->dirtyLo = t->dirtyHi = 0;
+    }
+    t->finalized = true;
+    return TPC_OK;
+}
+
+int stage_clusters(tpc_tracker* t, int64_t at, int64_t n, const float* y, const float* z) {
+    if (n == 0) return TPC_OK;
+    if (is_device_pointer(y)) {
+        CUDA_TRY(t, cudaMemcpyAsync((float*)t->dev.inY + at, y, sizeof(float) * n, cudaMemcpyDeviceToDevice, t->stream));
+        CUDA_TRY(t, cudaMemcpyAsync((float*)t->dev.inZ + at, z, sizeof(float) * n, cudaMemcpyDeviceToDevice, t->stream));
+    } else {
+        int rc = ensure_host_stage(t, at + n);
+        if (rc != TPC_OK) return rc;
+        std::memcpy(t->hostY + at, y, sizeof(float) * n);
+        std::memcpy(t->hostZ + at, z, sizeof(float) * n);
+        if (t->dirtyHi == t->dirtyLo) { t->dirtyLo = at; t->dirtyHi = at + n; }
+        else { t->dirtyLo = std::min(t->dirtyLo, at); t->dirtyHi = std::max(t->dirtyHi, at + n); }
+    }
+    return TPC_OK;
+}
+
+// ---- debug-dump conversion kernels (tests only; not on the hot path)
+__global__ void dump_links_kernel(DevPtrs d, int nRows, int64_t N, int32_t* out) {
+    const int rowId = blockIdx.x, r = rowId % nRows;
+    const RowInfo R = d.rows[rowId];
+    for (int k = threadIdx.x; k < R.n; k += blockDim.x) {
+        const int64_t g = (int64_t)R.gidBase + d.orig[R.hitOff + k];
+        const int32_t* src[4] = {d.linkUp, d.linkDn, d.linkUpC, d.linkDnC};
+        for (int w = 0; w < 4; w++) {
+            const int l = src[w][R.hitOff + k];
+            int v = -1;
+            if (l >= 0) {
+                const bool upw = (w % 2) == 0;
+                if ((upw && r + 1 < nRows) || (!upw && r >= 1)) v = (int)d.orig[d.rows[rowId + (upw ? 1 : -1)].hitOff + l];
+            }
+            out[(int64_t)w * N + g] = v;
+        }
+    }
+}
+__global__ void dump_starts_kernel(DevPtrs d, unsigned n, uint32_t* out) {
+    const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int2 s = d.starts[i];
+    const RowInfo R = d.rows[s.x];
+    out[i] = R.gidBase + d.orig[R.hitOff + s.y];
+}
+__global__ void dump_rowhit_kernel(DevPtrs d, int nRows, unsigned n, int32_t* out) {
+    const unsigned slot = blockIdx.x;
+    if (slot >= n) return;
+    const TrackletRec t = d.recs[slot];
+    for (int r = threadIdx.x; r < nRows; r += blockDim.x) {
+        int v = -1;
+        if (r >= t.firstRow && r <= t.lastRow) {
+            const int h = d.rowHit[(size_t)slot * d.rhStride + r];
+            if (h >= 0) v = (int)d.orig[d.rows[t.sector * nRows + r].hitOff + h];
+        }
+        out[(size_t)slot * nRows + r] = v;
+    }
+}
+__global__ void dump_owner_kernel(DevPtrs d, int nRows, uint32_t* out) {
+    const int rowId = blockIdx.x;
+    const RowInfo R = d.rows[rowId];
+    const uint32_t sb = d.sectorGidBase[rowId / nRows];
+    for (int k = threadIdx.x; k < R.n; k += blockDim.x) {
+        const uint32_t w = d.weight[R.hitOff + k];
+        out[R.gidBase + d.orig[R.hitOff + k]] = w ? sb + (0x00FFFFFFu - (w & 0x00FFFFFFu)) : 0xFFFFFFFFu;
+    }
+}
+
+}  // namespace
+
+extern "C" {
+
+void tpc_default_params(tpc_params* p) {
+    if (!p) return;
+    p->err2_y = 0.01f; p->err2_z = 0.01f;
+    p->nf_ty = 1.0f; p->nf_tz = 1.5f; p->nf_c = 0.5f; p->nf_d2max = 0.25f;
+    p->kf_css0 = 1.0f; p->kf_ctt0 = 10.0f; p->kf_ckk0 = 100.0f; p->kf_smax = 0.95f;
+    p->road_nsig = 4.0f; p->road_max = 2.0f;
+    p->max_gap = 4; p->min_hits = 10; p->seed_min_chain = 3;
+    p->max_tracklets_per_cluster = 0.125f;
+}
+
+int tpc_tracker_create(const tpc_geometry* g, float bz_tesla, tpc_tracker** out) {
+    if (!g || !out || !g->row_x) return TPC_E_ARG;
+    if (g->n_sectors < 1 || g->n_rows < 3 || g->n_rows > kMaxRows) return TPC_E_ARG;
+    if ((int64_t)g->n_sectors * g->n_rows > (1 << 24)) return TPC_E_ARG;
+    for (int i = 1; i < g->n_rows; i++)
+        if (!(g->row_x[i] > g->row_x[i - 1])) return TPC_E_ARG;
+    tpc_tracker* t = new (std::nothrow) tpc_tracker();
+    if (!t) return TPC_E_NOMEM;
+    t->nSec = g->n_sectors; t->nRows = g->n_rows; t->nRowsTotal = g->n_sectors * g->n_rows;
+    t->rhStride = (g->n_rows + 31) / 32 * 32;
+    t->rowX.assign(g->row_x, g->row_x + g->n_rows);
+    if (g->params) t->P = *g->params; else tpc_default_params(&t->P);
+    if (t->P.seed_min_chain < 2 || t->P.min_hits < 1 || t->P.max_gap < 0 || !(t->P.max_tracklets_per_cluster > 0.f)) {
+        delete t; return TPC_E_ARG;
+    }
+    t->bz = bz_tesla;
+    t->CB = (float)(-0.299792458e-2 * (double)bz_tesla);   // kappa = (q/pT) * CB, constant field
+    t->rowN.assign(t->nRowsTotal, 0); t->rowIn.assign(t->nRowsTotal, 0);
+    *out = t;
+    return TPC_OK;
+}
+
+void tpc_tracker_destroy(tpc_tracker* t) {
+    if (!t) return;
+    if (t->stream || t->ws) cudaStreamSynchronize(t->stream);
+    if (t->hostY) cudaFreeHost(t->hostY);
+    if (t->hostZ) cudaFreeHost(t->hostZ);
+    if (t->hostRows) cudaFreeHost(t->hostRows);
+    if (t->hostSectorBase) cudaFreeHost(t->hostSectorBase);
+    if (t->hostCounters) cudaFreeHost(t->hostCounters);
+    if (t->outTracks) cudaFreeHost(t->outTracks);
+    if (t->outIds) cudaFreeHost(t->outIds);
+    if (t->haveEvents) for (auto& e : t->ev) cudaEventDestroy(e);
+    delete t;
+}
+
+int tpc_set_stream(tpc_tracker* t, void* cuda_stream) {
+    if (!t) return TPC_E_ARG;
+    t->stream = (cudaStream_t)cuda_stream;
+    return TPC_OK;
+}
+
+size_t tpc_workspace_bytes(const tpc_tracker* t, int64_t max_clusters) {
+    if (!t || max_clusters < 0) return 0;
+    return make_layout(t, max_clusters).total;
+}
+
+int tpc_set_workspace(tpc_tracker* t, void* dev_ptr, size_t bytes) {
+    if (!t || !dev_ptr || ((uintptr_t)dev_ptr % kAlign) != 0) return TPC_E_ARG;
+    // capacity = largest max_clusters whose layout fits (the layout is monotone in max_clusters)
+    if (make_layout(t, 0).total > bytes) return TPC_E_NOMEM;
+    int64_t lo = 0, hi = 1;
+    while (make_layout(t, hi).total <= bytes && hi < (int64_t)1 << 31) hi *= 2;
+    while (hi - lo > 1) {
+        const int64_t mid = lo + (hi - lo) / 2;
+        if (make_layout(t, mid).total <= bytes) lo = mid; else hi = mid;
+    }
+    lo = std::min<int64_t>(lo, ((int64_t)1 << 31) - 65536);
+    t->ws = (char*)dev_ptr; t->wsBytes = bytes; t->maxClusters = lo;
+    t->L = make_layout(t, lo);
+    bind_pointers(t);
+    CUDA_TRY(t, cudaMemcpyAsync((void*)t->dev.rowX, t->rowX.data(), sizeof(float) * t->nRows, cudaMemcpyHostToDevice, t->stream));
+    CUDA_TRY(t, cudaStreamSynchronize(t->stream));
+    if (!t->haveEvents) {
+        for (auto& e : t->ev) CUDA_TRY(t, cudaEventCreate(&e));
+        t->haveEvents = true;
+        int dev = 0, sms = 0, occ5 = 0, occ6 = 0;
+        CUDA_TRY(t, cudaGetDevice(&dev));
+        CUDA_TRY(t, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        CUDA_TRY(t, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ5, k5_construct, kK5Threads, 0));
+        CUDA_TRY(t, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ6, k6_select, kK6Threads, 0));
+        t->k5Blocks = sms * std::max(1, occ5);
+        t->k6Blocks = sms * std::max(1, occ6);
+    }
+    return tpc_reset_event(t);
+}
+
+int tpc_reset_event(tpc_tracker* t) {
+    if (!t) return TPC_E_ARG;
+    std::fill(t->rowN.begin(), t->rowN.end(), 0);
+    std::fill(t->rowIn.begin(), t->rowIn.end(), 0);
+    t->cursor = 0; t->nClusters = 0; t->dirtyLo = t->dirtyHi = 0;
+    t->finalized = t->tracked = t->fetched = false;
+    return TPC_OK;
+}
+
+int tpc_load_clusters(tpc_tracker* t, int sector, int row, int n, const float* x, const float* y, const float* z) {
+    (void)x;   // R-13: the tracker uses the pad-row x
+    if (!t || sector < 0 || sector >= t->nSec || row < 0 || row >= t->nRows || n < 0) return TPC_E_ARG;
+    if (n > 0 && (!y || !z)) return TPC_E_ARG;
+    if (!t->ws) return TPC_E_STATE;
+    if (t->cursor + n > t->maxClusters) return TPC_E_NOMEM;
+    const int i = sector * t->nRows + row;
+    int rc = stage_clusters(t, t->cursor, n, y, z);
+    if (rc != TPC_OK) return rc;
+    t->rowN[i] = n; t->rowIn[i] = (int32_t)t->cursor;
+    t->cursor += n;
+    t->finalized = t->tracked = t->fetched = false;
+    return TPC_OK;
+}
+
+int tpc_load_event(tpc_tracker* t, const int32_t* row_counts, const float* y, const float* z) {
+    if (!t || !row_counts) return TPC_E_ARG;
+    if (!t->ws) return TPC_E_STATE;
+    int64_t total = 0;
+    for (int i = 0; i < t->nRowsTotal; i++) {
+        if (row_counts[i] < 0) return TPC_E_ARG;
+        total += row_counts[i];
+    }
+    if (total > 0 && (!y || !z)) return TPC_E_ARG;
+    if (total > t->maxClusters) return TPC_E_NOMEM;
+    tpc_reset_event(t);
+    int64_t off = 0;
+    for (int i = 0; i < t->nRowsTotal; i++) { t->rowN[i] = row_counts[i]; t->rowIn[i] = (int32_t)off; off += row_counts[i]; }
+    t->cursor = total;
+    int rc = stage_clusters(t, 0, total, y, z);
+    if (rc != TPC_OK) return rc;
+    return finalize_event(t);
+}
+
+int tpc_track_sectors(tpc_tracker* t) {
+    if (!t) return TPC_E_ARG;
+    if (!t->ws) return TPC_E_STATE;
+    int rc = finalize_event(t);
+    if (rc != TPC_OK) return rc;
+    const DevPtrs d = t->dev;
+    DevParams dp; dp.P = t->P; dp.CB = t->CB; dp.nSec = t->nSec; dp.nRows = t->nRows;
+    const int NR = t->nRowsTotal;
+    cudaStream_t s = t->stream;
+    CUDA_TRY(t, cudaEventRecord(t->ev[0], s));
+    k1_sort_grid<<<NR, kK1Threads, sizeof(uint32_t) * (t->maxBinsLaunch + 1), s>>>(d);
+    CUDA_TRY(t, cudaEventRecord(t->ev[1], s));
+    k2_neighbours<<<NR, kK2Threads, 0, s>>>(d, dp);
+    CUDA_TRY(t, cudaEventRecord(t->ev[2], s));
+    k3_clean_start<<<NR, kK3Threads, 0, s>>>(d, dp);
+    CUDA_TRY(t, cudaEventRecord(t->ev[3], s));
+    k5_construct<<<t->k5Blocks, kK5Threads, 0, s>>>(d, dp);
+    CUDA_TRY(t, cudaEventRecord(t->ev[4], s));
+    k6_weights<<<t->k6Blocks, kK6Threads, 0, s>>>(d, dp);
+    CUDA_TRY(t, cudaEventRecord(t->ev[5], s));
+    k6_select<<<t->k6Blocks, kK6Threads, 0, s>>>(d, dp);
+    CUDA_TRY(t, cudaEventRecord(t->ev[6], s));
+    CUDA_TRY(t, cudaGetLastError());
+    t->tracked = true; t->fetched = false;
+    return TPC_OK;
+}
+
+int tpc_launches_per_track(const tpc_tracker* t) { (void)t; return 6; }
+
+int tpc_sync(tpc_tracker* t) {
+    if (!t) return TPC_E_ARG;
+    if (!t->tracked) return TPC_E_STATE;
+    CUDA_TRY(t, cudaMemcpyAsync(t->hostCounters, t->dev.counters, sizeof(uint32_t) * kNCounters, cudaMemcpyDeviceToHost, t->stream));
+    CUDA_TRY(t, cudaStreamSynchronize(t->stream));
+    std::memcpy(t->counters, t->hostCounters, sizeof(t->counters));
+    float total = 0.f;
+    for (int i = 0; i < 6; i++) {
+        float ms = 0.f;
+        CUDA_TRY(t, cudaEventElapsedTime(&ms, t->ev[i], t->ev[i + 1]));
+        t->kernelUs[i] = ms * 1000.f;
+    }
+    CUDA_TRY(t, cudaEventElapsedTime(&total, t->ev[0], t->ev[6]));
+    t->kernelUs[6] = total * 1000.f; t->kernelUs[7] = 0.f;
+    return TPC_OK;
+}
+
+int tpc_get_tracks(tpc_tracker* t, const tpc_track** tracks, int32_t* n_tracks, const uint32_t** cluster_ids,
+                   int64_t* n_cluster_ids) {
+    if (!t || !tracks || !n_tracks || !cluster_ids || !n_cluster_ids) return TPC_E_ARG;
+    int rc = tpc_sync(t);
+    if (rc != TPC_OK) return rc;
+    const int64_t nT = t->counters[kNTracks], nC = t->counters[kNTrackClusters];
+    if (nT > t->outTracksCap) {
+        if (t->outTracks) cudaFreeHost(t->outTracks);
+        t->outTracksCap = std::max<int64_t>(nT, 1024) * 3 / 2;
+        CUDA_TRY(t, cudaMallocHost(&t->outTracks, sizeof(tpc_track) * t->outTracksCap));
+    }
+    if (nC > t->outIdsCap) {
+        if (t->outIds) cudaFreeHost(t->outIds);
+        t->outIdsCap = std::max<int64_t>(nC, 1024) * 3 / 2;
+        CUDA_TRY(t, cudaMallocHost(&t->outIds, sizeof(uint32_t) * t->outIdsCap));
+    }
+    if (nT) CUDA_TRY(t, cudaMemcpyAsync(t->outTracks, t->dev.tracks, sizeof(tpc_track) * nT, cudaMemcpyDeviceToHost, t->stream));
+    if (nC) CUDA_TRY(t, cudaMemcpyAsync(t->outIds, t->dev.clusterIds, sizeof(uint32_t) * nC, cudaMemcpyDeviceToHost, t->stream));
+    CUDA_TRY(t, cudaStreamSynchronize(t->stream));
+    *tracks = t->outTracks; *n_tracks = (int32_t)nT; *cluster_ids = t->outIds; *n_cluster_ids = nC;
+    t->fetched = true;
+    return t->counters[kNStart] > (uint32_t)t->dev.maxTracklets ? TPC_E_OVERFLOW : TPC_OK;
+}
+
+int tpc_get_stats(tpc_tracker* t, tpc_stats* out) {
+    if (!t || !out) return TPC_E_ARG;
+    std::memset(out, 0, sizeof(*out));
+    out->n_clusters = t->nClusters;
+    out->max_clusters = t->maxClusters;
+    out->max_tracklets = t->ws ? t->dev.maxTracklets : 0;
+    out->workspace_bytes_used = (int64_t)t->L.total;
+    if (!t->tracked) return TPC_OK;
+    out->n_links = t->counters[kNLinks];
+    out->n_start_hits = t->counters[kNStart];
+    out->n_tracklets = t->counters[kNKept];
+    out->n_tracklet_hits = t->counters[kHitsTotal];
+    out->n_tracks = t->counters[kNTracks];
+    out->n_track_clusters = t->counters[kNTrackClusters];
+    std::memcpy(out->kernel_us, t->kernelUs, sizeof(out->kernel_us));
+    return TPC_OK;
+}
+
+size_t tpc_debug_dump_bytes(tpc_tracker* t, int stage) {
+    if (!t || !t->tracked) return 0;
+    if (tpc_sync(t) != TPC_OK) return 0;
+    const size_t N = (size_t)t->nClusters;
+    const size_t M = std::min<size_t>(t->counters[kNStart], (size_t)t->dev.maxTracklets);
+    switch (stage) {
+        case TPC_DUMP_LINKS: return 4 * N * sizeof(int32_t);
+        case TPC_DUMP_START_HITS: return M * sizeof(uint32_t);
+        case TPC_DUMP_TRACKLETS: return M * (sizeof(tpc_tracklet) + sizeof(int32_t) * t->nRows);
+        case TPC_DUMP_OWNERS: return N * sizeof(uint32_t);
+        default: return 0;
+    }
+}
+
+int tpc_debug_dump(tpc_tracker* t, int stage, void* host_dst, size_t bytes) {
+    if (!t || (!host_dst && bytes)) return TPC_E_ARG;
+    if (!t->tracked) return TPC_E_STATE;
+    const size_t need = tpc_debug_dump_bytes(t, stage);
+    if (stage < TPC_DUMP_LINKS || stage > TPC_DUMP_OWNERS || bytes != need) return TPC_E_ARG;
+    if (need == 0) return TPC_OK;
+    const size_t N = (size_t)t->nClusters;
+    const unsigned M = (unsigned)std::min<size_t>(t->counters[kNStart], (size_t)t->dev.maxTracklets);
+    void* tmp = nullptr;
+    cudaStream_t s = t->stream;
+    int rc = TPC_OK;
+    auto fail = [&](cudaError_t e) { t->lastCuda = (int)e; rc = TPC_E_CUDA; };
+    cudaError_t e;
+    if (stage == TPC_DUMP_TRACKLETS) {
+        const size_t rhBytes = (size_t)M * t->nRows * sizeof(int32_t);
+        if ((e = cudaMalloc(&tmp, rhBytes)) != cudaSuccess) { fail(e); return rc; }
+        dump_rowhit_kernel<<<M, 64, 0, s>>>(t->dev, t->nRows, M, (int32_t*)tmp);
+        std::vector<TrackletRec> recs(M);
+        if ((e = cudaMemcpyAsync(recs.data(), t->dev.recs, sizeof(TrackletRec) * M, cudaMemcpyDeviceToHost, s)) != cudaSuccess) fail(e);
+        char* dst = (char*)host_dst;
+        if (rc == TPC_OK && (e = cudaMemcpyAsync(dst + sizeof(tpc_tracklet) * M, tmp, rhBytes, cudaMemcpyDeviceToHost, s)) != cudaSuccess) fail(e);
+        if ((e = cudaStreamSynchronize(s)) != cudaSuccess) fail(e);
+        if (rc == TPC_OK) {
+            tpc_tracklet* o = (tpc_tracklet*)dst;
+            for (unsigned i = 0; i < M; i++) {
+                const TrackletRec& r = recs[i];
+                o[i].start_gid = r.startGid; o[i].sector = r.sector; o[i].start_row = r.startRow; o[i].n_hits = r.nHits;
+                o[i].first_row = r.firstRow; o[i].last_row = r.lastRow; o[i].n_fit = r.nFit;
+                o[i].x = (r.xRow >= 0 && r.xRow < t->nRows) ? t->rowX[r.xRow] : 0.f;
+                std::memcpy(o[i].p, r.p, sizeof(r.p)); std::memcpy(o[i].c, r.c, sizeof(r.c)); o[i].chi2 = r.chi2;
+            }
+        }
+    } else {
+        if ((e = cudaMalloc(&tmp, need)) != cudaSuccess) { fail(e); return rc; }
+        if (stage == TPC_DUMP_LINKS) dump_links_kernel<<<t->nRowsTotal, 128, 0, s>>>(t->dev, t->nRows, (int64_t)N, (int32_t*)tmp);
+        else if (stage == TPC_DUMP_START_HITS) dump_starts_kernel<<<(M + 127) / 128, 128, 0, s>>>(t->dev, M, (uint32_t*)tmp);
+        else dump_owner_kernel<<<t->nRowsTotal, 128, 0, s>>>(t->dev, t->nRows, (uint32_t*)tmp);
+        if ((e = cudaMemcpyAsync(host_dst, tmp, need, cudaMemcpyDeviceToHost, s)) != cudaSuccess) fail(e);
+        if ((e = cudaStreamSynchronize(s)) != cudaSuccess) fail(e);
+    }
+    if ((e = cudaGetLastError()) != cudaSuccess) fail(e);
+    cudaFree(tmp);
+    return rc;
+}
+
+const char* tpc_strerror(int code) {
+    switch (code) {
+        case TPC_OK: return "ok";
+        case TPC_E_ARG: return "invalid argument";
+        case TPC_E_STATE: return "call out of order";
+        case TPC_E_NOMEM: return "workspace too small";
+        case TPC_E_OVERFLOW: return "tracklet capacity exceeded";
+        case TPC_E_CUDA: return "CUDA error or no device";
+        default: return "unknown error";
+    }
+}
+
+int tpc_last_cuda_error(const tpc_tracker* t) { return t ? t->lastCuda : 0; }
+
+}  // extern "C"
