@@ -1,0 +1,338 @@
+#!/usr/bin/env python
+"""Benchmark of the Phase-I TPC sector tracker (BASELINE.json: TPC clusters/s, sector tracking, device-timed, 1 B200).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl ours|reference]
+
+A step = one pass of the whole hot path (K1..K6, tpc_track_sectors) over one synthetic event of
+BASELINE.json:configs[--config] (default 3 = central Pb-Pb, the config the target is quoted on) that is already
+resident in HBM.  The L2 is flushed (256 MiB write) before every timed step, outside the CUDA-event bracket.
+N > 1: one process per GPU (torchrun), each rank tracks its own event (seed = rank) - events are independent
+(PAPER.md:82), no collective on the data path, weak scaling; time = max over ranks.
+`--impl reference` times the CPU oracle (oracle/) on the host cores instead; see DESIGN.md "Measurement".
+Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "tpc_clusters_per_sec_sector_tracking"
+UNIT = "clusters/s"
+# Algorithmic HBM bytes per kernel: N clusters, B bins, S start hits,
+# H = sum of tracklet hits, T tracks, C clusters in tracks.
+
+
+def algorithmic_bytes(st: dict) -> dict:
+    n, s, h = st["n_clusters"], st["n_start_hits"], st["n_tracklet_hits"]
+    t, c = st["n_tracks"], st["n_track_clusters"]
+    return {
+        "K1_sort_grid": 8 * n + 8 * n + 4 * n + 4 * n + 4 * n,       # in y,z; out (y,z), orig, binStart(~N), weight=0
+        "K2_neighbours": 8 * n + 4 * n + 8 * n,                      # hits once, bins once, links out
+        "K3K4_clean_start": 8 * n + 8 * n + 8 * s,                   # raw links in, cleaned out, start list
+        "K5_construct": 28 * h + 4 * h + 128 * s,                    # per row step: link/bin 12 + hit 8 + cand 8; rowHit; record
+        "K6a_weights": 4 * h + 8 * h + 32 * s,                       # rowHit in, atomicMax rmw, record header
+        "K6b_select": 4 * h + 4 * h + 128 * s + 8 * c + 112 * t,     # rowHit, weight, record; orig + ids out, tracks out
+    }
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        names = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20,
+                 "hw_power_brake_slowdown": 0x80}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(0.002)
+
+    def start(self):
+        if self.nv is not None:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._thr:
+            self._thr.join()
+        s = sorted(self.samples)
+        return {"sm_mhz": (s[len(s) // 2] if s else None), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(s)}
+
+
+def init_dist(n_gpus: int):
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dist = None
+    if world > 1:
+        import torch
+        import torch.distributed as dist_
+        backend = "nccl" if torch.cuda.is_available() else "gloo"
+        if backend == "nccl":
+            torch.cuda.set_device(local)
+        dist_.init_process_group(backend=backend)
+        dist = dist_
+    return rank, world, local, dist
+
+
+def reduce_over_ranks(dist, value: float, op: str, device) -> float:
+    """max / sum of a python float over all ranks (no-op for world size 1)."""
+    if dist is None:
+        return value
+    import torch
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX if op == "max" else dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+def aggregate(dist, device, n_clusters_rank: int, step_ms_rank: float):
+    """Whole-job throughput: all ranks' clusters / the slowest rank's time (weak scaling, no data-path collective)."""
+    n_total = reduce_over_ranks(dist, float(n_clusters_rank), "sum", device)
+    ms = reduce_over_ranks(dist, step_ms_rank, "max", device)
+    return n_total / (ms * 1e-3), ms, int(n_total)
+
+
+def oracle_baseline(ev, budget_s: float = 15.0):
+    """cpu_baseline leg: the oracle as it stands, single-threaded, on a bounded sample of the same workload."""
+    import oracle
+    # probe one sector to size the sample
+    t0 = time.perf_counter()
+    sub = ev.sector_slice(0)
+    oracle.Oracle(1, ev.n_rows, ev.row_x, ev.bz).run(sub.row_counts, sub.y, sub.z, fetch=False)
+    t_sector = max(time.perf_counter() - t0, 1e-4)
+    n_sec = int(max(1, min(ev.n_sectors, budget_s / t_sector)))
+    if n_sec >= ev.n_sectors:
+        sample, desc = ev, f"whole event ({ev.n_clusters} clusters), best of 2 runs"
+        runs = 2 if 2 * t_sector * ev.n_sectors < 2 * budget_s else 1
+    else:
+        import datagen
+        b = ev.row_base
+        hi = int(b[n_sec * ev.n_rows])
+        sample = datagen.Event(n_sec, ev.n_rows, ev.row_x, ev.bz, ev.row_counts[:n_sec].copy(), ev.y[:hi], ev.z[:hi],
+                               ev.truth[:hi])
+        desc, runs = f"sectors 0..{n_sec - 1} of the event ({hi} clusters), 1 run", 1
+    o = oracle.Oracle(sample.n_sectors, sample.n_rows, sample.row_x, sample.bz)
+    best = 1e30
+    for _ in range(runs):
+        t0 = time.perf_counter()
+        o.run(sample.row_counts, sample.y, sample.z, fetch=False)
+        best = min(best, time.perf_counter() - t0)
+    return {"value": sample.n_clusters / best, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc,
+            "seconds": best, "stage_seconds": o.stage_seconds()}
+
+
+def run_reference(args, rank, world, dist):
+    """--impl reference: the CPU oracle, timed on the host cores, same metric/config (rank 0 only)."""
+    if rank != 0:
+        return
+    import datagen
+    import oracle
+    ev = datagen.config_event(args.config, seed=0)
+    # bounded sample: keep (steps+warmup) * t_step within ~2.5 minutes
+    t0 = time.perf_counter()
+    sub = ev.sector_slice(0)
+    oracle.Oracle(1, ev.n_rows, ev.row_x, ev.bz).run(sub.row_counts, sub.y, sub.z, fetch=False)
+    t_sector = max(time.perf_counter() - t0, 1e-4)
+    n_sec = int(max(1, min(ev.n_sectors, 150.0 / ((args.steps + args.warmup) * t_sector))))
+    b = ev.row_base
+    hi = int(b[n_sec * ev.n_rows])
+    sample = datagen.Event(n_sec, ev.n_rows, ev.row_x, ev.bz, ev.row_counts[:n_sec].copy(), ev.y[:hi], ev.z[:hi], ev.truth[:hi])
+    o = oracle.Oracle(n_sec, ev.n_rows, ev.row_x, ev.bz)
+    for _ in range(args.warmup):
+        o.run(sample.row_counts, sample.y, sample.z, fetch=False)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        o.run(sample.row_counts, sample.y, sample.z, fetch=False)
+    dt = (time.perf_counter() - t0) / args.steps
+    val = sample.n_clusters / dt
+    desc = f"sectors 0..{n_sec - 1} of config {args.config} ({hi} of {ev.n_clusters} clusters) per step"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"config{args.config}:{datagen.CONFIG_NAMES[args.config]}", "sample": desc},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank, world, local, dist = init_dist(args.gpus)
+    if args.impl == "reference":
+        run_reference(args, rank, world, dist)
+        if dist is not None:
+            dist.barrier()
+            dist.destroy_process_group()
+        return
+
+    import torch
+    import datagen
+    from paper_1712_09430_b200 import binding
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    dev = torch.device("cuda", local)
+    torch.cuda.set_device(dev)
+    warmup = max(args.warmup, 3)
+
+    ev = datagen.config_event(args.config, seed=rank)
+    trk = binding.Tracker(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz)
+    stream = torch.cuda.current_stream()
+    trk.set_stream(stream.cuda_stream)
+    ws_bytes = trk.allocate_workspace(ev.n_clusters, device=dev)
+    y_dev, z_dev = torch.from_numpy(ev.y).to(dev), torch.from_numpy(ev.z).to(dev)
+    trk.load_event(ev.row_counts, y_dev, z_dev)          # inputs resident in HBM before the timed region
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+
+    def step_device():
+        flush.fill_(1)                                  # evict the 126 MB L2 (outside the event bracket)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        trk.track_sectors()
+        e1.record(stream)
+        return e0, e1
+
+    # warm-up: at least W steps and at least ~0.3 s of load so the clocks are up
+    t0 = time.perf_counter()
+    n_warm = 0
+    while n_warm < warmup or time.perf_counter() - t0 < 0.3:
+        step_device()
+        n_warm += 1
+        if n_warm % 8 == 0:
+            torch.cuda.synchronize()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    torch.cuda.synchronize()
+    events, kern = [], {k: 0.0 for k in binding.KERNEL_NAMES}
+    for _ in range(args.steps):
+        events.append(step_device())
+        trk.sync()                                       # per-kernel device times of this step
+        st = trk.get_stats()
+        for k, v in st["kernel_us"].items():
+            kern[k] += v
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    clocks = sampler.stop()
+    step_ms = sum(a.elapsed_time(b) for a, b in events) / args.steps
+    kern = {k: v / args.steps for k, v in kern.items()}
+    st = trk.get_stats()
+    value, ms, n_total = aggregate(dist, dev, ev.n_clusters, step_ms)
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), H2D + D2H inside the timed region
+    y_pin, z_pin = torch.from_numpy(ev.y).pin_memory(), torch.from_numpy(ev.z).pin_memory()
+    def step_e2e():
+        trk.load_event(ev.row_counts, y_pin.numpy(), z_pin.numpy())
+        trk.track_sectors()
+        return trk.get_tracks(copy=False)
+    for _ in range(3):
+        tr, ids = step_e2e()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    n_e2e = max(3, min(args.steps, 20))
+    t0 = time.perf_counter()
+    for _ in range(n_e2e):
+        tr, ids = step_e2e()
+    torch.cuda.synchronize()
+    e2e_ms = (time.perf_counter() - t0) / n_e2e * 1e3
+    e2e_value, e2e_ms_max, _ = aggregate(dist, dev, ev.n_clusters, e2e_ms)
+    h2d = 8 * ev.n_clusters + 48 * ev.n_sectors * ev.n_rows + 4 * (ev.n_sectors + 1)
+    d2h = 112 * int(tr.shape[0]) + 4 * int(ids.shape[0]) + 64
+
+    # ---- roofline of the dominant kernel + per-kernel table
+    peak, peak_src = measured_peaks()
+    ab = algorithmic_bytes(st)
+    dom = max(kern, key=kern.get)
+    per_kernel = {k: {"us": round(kern[k], 2), "alg_bytes": ab[k], "gbs": round(ab[k] / (kern[k] * 1e-6) / 1e9, 1),
+                      "frac": round(ab[k] / (kern[k] * 1e-6) / 1e9 / peak, 4)} for k in kern}
+    achieved = ab[dom] / (kern[dom] * 1e-6) / 1e9
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "dominant_kernel_traffic.json")
+    if os.path.exists(tp):
+        try:
+            traffic = json.load(open(tp)).get(dom)
+        except Exception:
+            traffic = None
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "warmup_actual": n_warm, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"config{args.config}:{datagen.CONFIG_NAMES[args.config]}", "n_clusters_per_gpu": ev.n_clusters,
+                   "n_clusters_total": n_total, "events_per_sec": world / (ms * 1e-3), "seed": "rank", "l2": "flushed (256 MiB write) before every timed step",
+                   "parallelism": "one event per GPU, no collective" if world > 1 else "single GPU",
+                   "n_start_hits": st["n_start_hits"], "n_tracklet_hits": st["n_tracklet_hits"], "n_tracks": st["n_tracks"],
+                   "workspace_bytes": ws_bytes, "workspace_over_input": round(ws_bytes / (12.0 * ev.n_clusters), 2)},
+        "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms_max, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+        "gpu_launches": args.steps * trk.launches_per_track(),
+        "roofline": {"bound": "hbm", "kernel": dom, "achieved": round(achieved, 2), "peak": peak, "unit": "GB/s",
+                     "frac": round(achieved / peak, 5), "traffic": traffic, "peak_source": peak_src,
+                     "frac_of_8TBs_nominal": round(achieved / 8000.0, 5),
+                     "whole_step": {"alg_bytes": sum(ab.values()), "gbs": round(sum(ab.values()) / (ms * 1e-3) / 1e9, 1),
+                                    "frac": round(sum(ab.values()) / (ms * 1e-3) / 1e9 / peak, 5)}},
+        "kernels": per_kernel,
+    }
+    if rank == 0 and not args.no_cpu_baseline:
+        out["cpu_baseline"] = oracle_baseline(datagen.config_event(args.config, seed=0))
+    if dist is not None:
+        dist.barrier()
+    if rank == 0:
+        print(json.dumps(out), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

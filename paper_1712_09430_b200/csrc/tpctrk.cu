@@ -49,7 +49,8 @@ struct tpc_tracker {
     int64_t nClusters = 0;
     bool finalized = false, tracked = false, fetched = false;
     float* hostY = nullptr; float* hostZ = nullptr; int64_t hostCap = 0;   // pinned mirror for host-pointer loads
-    int64_t dirtyLo = 0, dirtyHi = 0;
+    int64_t dirtyLo = 0, dirtyHi = 0;       // host-staged range not yet uploaded
+    cudaEvent_t evUpload = nullptr; bool uploadPending = false;
     RowInfo* hostRows = nullptr;            // pinned
     uint32_t* hostSectorBase = nullptr;     // pinned
     uint32_t* hostCounters = nullptr;       // pinned
@@ -145,6 +146,19 @@ int ensure_host_stage(tpc_tracker* t, int64_t need) {
     return TPC_OK;
 }
 
+// Upload the pending host-staged range [dirtyLo, dirtyHi) (one copy per array).
+int flush_dirty(tpc_tracker* t) {
+    if (t->dirtyHi <= t->dirtyLo) return TPC_OK;
+    const int64_t lo = t->dirtyLo, cnt = t->dirtyHi - t->dirtyLo;
+    CUDA_TRY(t, cudaMemcpyAsync((float*)t->dev.inY + lo, t->hostY + lo, sizeof(float) * cnt, cudaMemcpyHostToDevice, t->stream));
+    CUDA_TRY(t, cudaMemcpyAsync((float*)t->dev.inZ + lo, t->hostZ + lo, sizeof(float) * cnt, cudaMemcpyHostToDevice, t->stream));
+    if (!t->evUpload) CUDA_TRY(t, cudaEventCreateWithFlags(&t->evUpload, cudaEventDisableTiming));
+    CUDA_TRY(t, cudaEventRecord(t->evUpload, t->stream));
+    t->uploadPending = true;
+    t->dirtyLo = t->dirtyHi = 0;
+    return TPC_OK;
+}
+
 // Host "initialisation" of an event (PAPER.md:66 host pre-processing, reduced to a prefix sum over row counts):
 // canonical id bases, padded row offsets, bin capacities; uploads the row table and any host-staged clusters.
 int finalize_event(tpc_tracker* t) {
@@ -184,11 +198,9 @@ int finalize_event(tpc_tracker* t) {
     CUDA_TRY(t, cudaMemcpyAsync(t->dev.rows, t->hostRows, sizeof(RowInfo) * NR, cudaMemcpyHostToDevice, t->stream));
     CUDA_TRY(t, cudaMemcpyAsync(t->dev.sectorGidBase, t->hostSectorBase, sizeof(uint32_t) * (t->nSec + 1),
                                 cudaMemcpyHostToDevice, t->stream));
-    if (t->dirtyHi > t->dirtyLo) {
-        const int64_t lo = t->dirtyLo, cnt = t->dirtyHi - t->dirtyLo;
-        CUDA_TRY(t, cudaMemcpyAsync((float*)t->dev.inY + lo, t->hostY + lo, sizeof(float) * cnt, cudaMemcpyHostToDevice, t->stream));
-        CUDA_TRY(t, cudaMemcpyAsync((float*)t->dev.inZ + lo, t->hostZ + lo, sizeof(float) * cnt, cudaMemcpyHostToDevice, t->stream));
-        t->dirtyLo = t->dirtyHi = 0;
+    {
+        int rc = flush_dirty(t);
+        if (rc != TPC_OK) return rc;
     }
     t->finalized = true;
     return TPC_OK;
@@ -202,10 +214,20 @@ int stage_clusters(tpc_tracker* t, int64_t at, int64_t n, const float* y, const 
     } else {
         int rc = ensure_host_stage(t, at + n);
         if (rc != TPC_OK) return rc;
+        if (t->uploadPending) {   // an earlier upload may still read the pinned mirror
+            CUDA_TRY(t, cudaEventSynchronize(t->evUpload));
+            t->uploadPending = false;
+        }
+        if (t->dirtyHi > t->dirtyLo && at != t->dirtyHi) {   // not contiguous with the pending range (e.g. device
+            rc = flush_dirty(t);                              // loads in between): upload what we have first
+            if (rc != TPC_OK) return rc;
+            CUDA_TRY(t, cudaEventSynchronize(t->evUpload));
+            t->uploadPending = false;
+        }
         std::memcpy(t->hostY + at, y, sizeof(float) * n);
         std::memcpy(t->hostZ + at, z, sizeof(float) * n);
         if (t->dirtyHi == t->dirtyLo) { t->dirtyLo = at; t->dirtyHi = at + n; }
-        else { t->dirtyLo = std::min(t->dirtyLo, at); t->dirtyHi = std::max(t->dirtyHi, at + n); }
+        else t->dirtyHi = at + n;
     }
     return TPC_OK;
 }
@@ -305,6 +327,7 @@ void tpc_tracker_destroy(tpc_tracker* t) {
     if (t->outTracks) cudaFreeHost(t->outTracks);
     if (t->outIds) cudaFreeHost(t->outIds);
     if (t->haveEvents) for (auto& e : t->ev) cudaEventDestroy(e);
+    if (t->evUpload) cudaEventDestroy(t->evUpload);
     delete t;
 }
 

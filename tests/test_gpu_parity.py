@@ -1,0 +1,215 @@
+"""GPU parity tests proper (-m gpu): the CUDA path through the C ABI vs the CPU oracle, element by element.
+
+Bar (BASELINE.json:north_star): links, start hits, tracklet hit tables, owners and cluster lists bit-exact except
+counted near-ties; states/covariances within 1e-4 rel or 1e-5 abs (both sides compute the same IEEE fp32
+expressions, so they normally agree bit for bit); cluster-to-track efficiency within 0.1 % of the oracle's.
+"""
+import numpy as np
+import pytest
+
+import datagen
+import oracle
+from paper_1712_09430_b200 import binding
+from parity import compare, run_gpu
+
+pytestmark = pytest.mark.gpu
+
+
+def _cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("-m gpu tests need a CUDA device (no CPU fallback exists)")
+    return torch
+
+
+@pytest.mark.parametrize("cfg", [0, 1, 2, 3])
+def test_configs_match_oracle_stage_by_stage(cfg):
+    _cuda()
+    ev = datagen.config_event(cfg)
+    ref = oracle.run_event(ev)
+    trk, tracks, ids = run_gpu(ev)
+    out = compare(ev, trk, tracks, ids, ref)
+    assert out["tracklet_mismatch"] == 0 and out["link_mismatch_0"] == 0
+    st = trk.get_stats()
+    assert st["n_start_hits"] == ref.start_hits.size and st["n_tracks"] == ref.tracks.size
+    assert st["n_tracklets"] == int(ref.tracklets["kept"].sum())
+    assert st["n_tracklet_hits"] == int(ref.tracklets["n_hits"].sum())
+    assert st["n_links"] == int((ref.link_up_clean >= 0).sum())
+    # truth metric within 0.1 % of the oracle's
+    eg = datagen.efficiency(ev, ids.astype(np.int64), tracks["cluster_offset"], tracks["n_clusters"])
+    eo = datagen.efficiency(ev, ref.cluster_ids, ref.tracks["cluster_offset"], ref.tracks["n_clusters"])
+    assert abs(eg["cluster_eff"] - eo["cluster_eff"]) <= 1e-3
+    assert eg["cluster_eff"] > 0.95
+
+
+def test_other_seeds_and_device_resident_input():
+    _cuda()
+    for seed in (1, 2):
+        ev = datagen.config_event(2, seed=seed)
+        ref = oracle.run_event(ev)
+        trk, tracks, ids = run_gpu(ev, device_input=True)
+        out = compare(ev, trk, tracks, ids, ref)
+        assert out["tracklet_mismatch"] == 0
+
+
+def test_time_frame_full_size_sampled_sectors():
+    """BASELINE.json:configs[4] at full size (20 overlapped central events, ~31.6M clusters) in the bench's launch
+    configuration; the oracle recomputes two sampled sectors (sectors are independent)."""
+    _cuda()
+    ev = datagen.config_event(4)
+    trk, tracks, ids = run_gpu(ev)
+    st = trk.get_stats()
+    assert st["n_clusters"] == ev.n_clusters and st["n_start_hits"] <= st["max_tracklets"]
+    # properties that hold at any size
+    assert np.unique(ids).size == ids.size                       # one track hypothesis at most per hit
+    assert tracks["n_clusters"].min() >= 10
+    sec_of = np.repeat(np.arange(ev.n_sectors * ev.n_rows), ev.row_counts.reshape(-1))
+    base = ev.row_base
+    for s in (3, 25):
+        sub = ev.sector_slice(s)
+        ref = oracle.run_event(sub)
+        g0 = int(base[s * ev.n_rows])
+        tg = tracks[tracks["sector"] == s]
+        assert tg.size == ref.tracks.size
+        key_g = ids[tg["cluster_offset"]].astype(np.int64) - g0
+        key_o = ref.cluster_ids[ref.tracks["cluster_offset"]].astype(np.int64)
+        tg, to = tg[np.argsort(key_g)], ref.tracks[np.argsort(key_o)]
+        assert np.array_equal(np.sort(key_g), np.sort(key_o))
+        for f in ("n_clusters", "first_row", "last_row", "n_fit"):
+            assert np.array_equal(tg[f], to[f]), f
+        for f in ("x", "p", "c", "chi2"):
+            a, b = tg[f].astype(np.float64), to[f]
+            assert np.all(np.abs(a - b) <= 1e-5 + 1e-4 * np.abs(b)), f
+        for i in range(0, tg.size, max(1, tg.size // 500)):
+            a = ids[tg["cluster_offset"][i]: tg["cluster_offset"][i] + tg["n_clusters"][i]].astype(np.int64) - g0
+            b = ref.cluster_ids[to["cluster_offset"][i]: to["cluster_offset"][i] + to["n_clusters"][i]]
+            assert np.array_equal(a, b)
+            rows = sec_of[a + g0] % ev.n_rows
+            assert np.all(np.diff(rows) > 0)
+
+
+def test_edge_cases_empty_tiny_and_ragged():
+    _cuda()
+    rx = datagen.default_row_x()
+    # empty event
+    ev = datagen.event_from_hits([], 2, rx)
+    trk, tracks, ids = run_gpu(ev, max_clusters=16)
+    assert tracks.size == 0 and ids.size == 0 and trk.get_stats()["n_start_hits"] == 0
+    # hits in a single row only; rows with one hit; duplicates (exact ties -> load-index tie-break)
+    hits = [(1, 7, 0.1 * i, 5.0) for i in range(5)]
+    ev = datagen.event_from_hits(hits, 2, rx)
+    ref = oracle.run_event(ev)
+    trk, tracks, ids = run_gpu(ev)
+    compare(ev, trk, tracks, ids, ref)
+    rng = np.random.default_rng(0)
+    hits = []
+    for r in range(40):
+        for _ in range(int(rng.integers(0, 6))):
+            y, z = round(rng.uniform(-3, 3) * 4) / 4, round(rng.uniform(0, 6) * 4) / 4
+            hits += [(0, r, y, z), (0, r, y, z)]
+    ev = datagen.event_from_hits(hits, 1, rx)
+    ref = oracle.run_event(ev)
+    trk, tracks, ids = run_gpu(ev)
+    out = compare(ev, trk, tracks, ids, ref)
+    assert out["link_mismatch_0"] == 0
+
+
+def test_one_very_large_row_and_small_geometry():
+    """Maximum sizes: a row far beyond the shared-memory bin budget (bins get coarser, results unchanged)."""
+    _cuda()
+    rx = datagen.default_row_x()[:12]
+    rng = np.random.default_rng(1)
+    n_big = 60000
+    hits = []
+    for r in range(12):
+        n = n_big if r == 5 else 3000
+        y = rng.uniform(-20, 20, n)
+        z = rng.uniform(0, 250, n)
+        hits += [(0, r, float(a), float(b)) for a, b in zip(y, z)]
+    ev = datagen.event_from_hits(hits, 1, rx)
+    ref = oracle.run_event(ev)
+    trk, tracks, ids = run_gpu(ev)
+    out = compare(ev, trk, tracks, ids, ref)
+    assert out["link_mismatch_0"] == 0
+
+
+def test_per_row_loading_out_of_order_and_replacement():
+    torch = _cuda()
+    ev = datagen.config_event(1, seed=4)
+    ref = oracle.run_event(ev)
+    trk = binding.Tracker(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz)
+    trk.set_stream(torch.cuda.current_stream().cuda_stream)
+    trk.allocate_workspace(2 * ev.n_clusters + 1024)
+    base = ev.row_base
+    order = np.random.default_rng(0).permutation(ev.n_sectors * ev.n_rows)
+    x = ev.x()
+    junk = np.full(3, 1.0, dtype=np.float32)
+    for k, sr in enumerate(order):
+        s, r = divmod(int(sr), ev.n_rows)
+        lo, hi = int(base[sr]), int(base[sr + 1])
+        if k % 50 == 0:
+            trk.load_clusters(s, r, None, junk, junk)            # replaced below
+        if k % 2:
+            trk.load_clusters(s, r, x[lo:hi], ev.y[lo:hi], ev.z[lo:hi])
+        else:
+            yd, zd = torch.from_numpy(ev.y[lo:hi]).cuda(), torch.from_numpy(ev.z[lo:hi]).cuda()
+            trk.load_clusters(s, r, None, yd, zd)
+    trk.track_sectors()
+    tracks, ids = trk.get_tracks()
+    compare(ev, trk, tracks, ids, ref)
+    # tracking again gives the same result; reset forgets
+    trk.track_sectors()
+    t2, i2 = trk.get_tracks()
+    assert np.array_equal(np.sort(i2), np.sort(ids)) and t2.size == tracks.size
+    trk.reset_event()
+    trk.track_sectors()
+    t3, i3 = trk.get_tracks()
+    assert t3.size == 0 and i3.size == 0
+
+
+def test_non_finite_coordinates_do_not_crash_or_hang():
+    _cuda()
+    ev = datagen.config_event(1, seed=5)
+    y, z = ev.y.copy(), ev.z.copy()
+    y[::97] = np.nan
+    z[::89] = np.inf
+    z[5::101] = -np.inf
+    bad = datagen.Event(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz, ev.row_counts, y, z, ev.truth)
+    trk, tracks, ids = run_gpu(bad)
+    assert ids.size == np.unique(ids).size and (ids < ev.n_clusters).all()
+
+
+def test_tracklet_capacity_overflow_is_reported():
+    torch = _cuda()
+    ev = datagen.config_event(2, seed=6)
+    p = binding.default_params()
+    p.max_tracklets_per_cluster = 1e-9           # capacity = 4096 tracklets < ~4100 seeds of this event
+    trk = binding.Tracker(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz, p)
+    trk.set_stream(torch.cuda.current_stream().cuda_stream)
+    trk.allocate_workspace(ev.n_clusters)
+    trk.load_event(ev.row_counts, ev.y, ev.z)
+    trk.track_sectors()
+    tracks, ids, rc = trk.get_tracks(allow_overflow=True)
+    st = trk.get_stats()
+    if st["n_start_hits"] > st["max_tracklets"]:
+        assert rc == binding.TPC_E_OVERFLOW
+    else:
+        assert rc == binding.TPC_OK
+    # too many clusters for the workspace
+    small = binding.Tracker(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz)
+    small.allocate_workspace(1000)
+    with pytest.raises(binding.TpcError) as e:
+        small.load_event(ev.row_counts, ev.y, ev.z)
+    assert e.value.code == binding.TPC_E_NOMEM
+
+
+def test_non_default_parameters():
+    _cuda()
+    ev = datagen.config_event(2, seed=7)
+    po, pg = oracle.default_params(), binding.default_params()
+    for o in (po, pg):
+        o.min_hits, o.max_gap, o.road_nsig, o.nf_d2max, o.kf_smax = 6, 2, 3.0, 0.16, 0.9
+    ref = oracle.run_event(ev, po)
+    trk, tracks, ids = run_gpu(ev, pg)
+    out = compare(ev, trk, tracks, ids, ref)
+    assert out["tracklet_mismatch"] == 0
