@@ -19,7 +19,8 @@
  * single-track events found with all clusters.  No function here is "parity unpinned".
  *
  * Templated on the scalar type: double for the 1e-5 self-checks, float for GPU parity
- * (build with -O2 -ffp-contract=off: IEEE fp32, no FMA contraction; R-12).
+ * (build with -O2 -ffp-contract=off: IEEE fp32; a fused multiply-add happens exactly where std::fma is written,
+ * nowhere else; R-12).
  */
 #include <algorithm>
 #include <chrono>
@@ -56,25 +57,24 @@ template <class T> bool propagate(State<T> &st, T x2, T CB, T smax, T (*Jout)[5]
     const T y = st.p[0], z = st.p[1], s = st.p[2], t = st.p[3], k = st.p[4];
     const T dx = x2 - st.x;
     const T kap = k * CB;
-    const T s2 = s + kap * dx;
+    const T s2 = std::fma(kap, dx, s);
     if (!(std::fabs(s) < smax) || !(std::fabs(s2) < smax)) return false;
-    const T c = std::sqrt(T(1) - s * s);
-    const T c2 = std::sqrt(T(1) - s2 * s2);
+    const T c = std::sqrt(std::fma(-s, s, T(1)));
+    const T c2 = std::sqrt(std::fma(-s2, s2, T(1)));
     const T cc = c + c2;
     const T ss = s + s2;
     const T rcc = T(1) / cc;
     const T tg = ss * rcc;                      /* tan of the mean direction */
-    const T q = std::sqrt(T(1) + tg * tg);
-    const T dy = dx * tg;
+    const T q = std::sqrt(std::fma(tg, tg, T(1)));
     const T l = dx * q;                         /* signed chord */
     const T a = (T(0.5) * kap) * l;
     const T a2 = a * a;
     const T c16 = T(1) / T(6), c340 = T(3) / T(40);
-    const T dS = l * (T(1) + a2 * (c16 + a2 * c340)); /* arc = chord * asin(a)/a, series */
+    const T dS = l * std::fma(a2, std::fma(a2, c340, c16), T(1)); /* arc = chord * asin(a)/a, series */
     const T rc = T(1) / c, rc2 = T(1) / c2;
     const T rcc2 = rcc * rcc;
-    const T d1 = ((ss * s) * rc + cc) * rcc2;   /* d tg / d s  */
-    const T d2 = ((ss * s2) * rc2 + cc) * rcc2; /* d tg / d s2 */
+    const T d1 = std::fma(ss * s, rc, cc) * rcc2;   /* d tg / d s  */
+    const T d2 = std::fma(ss * s2, rc2, cc) * rcc2; /* d tg / d s2 */
     T J[5][5];
     for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) J[i][j] = (i == j) ? T(1) : T(0);
     J[0][2] = dx * (d1 + d2);
@@ -83,29 +83,29 @@ template <class T> bool propagate(State<T> &st, T x2, T CB, T smax, T (*Jout)[5]
     const T rq = T(1) / q;
     const T sm = tg * rq;                       /* = dy/l; d l / d tg = dx*sm, so d l / d s = sm*J[y][s] */
     const T tsm = t * sm;
-    const T h = T(1) + a2 * (T(0.5) + a2 * T(0.375));   /* d dS / d l at fixed curvature */
-    const T gp = c16 + a2 * (T(3) / T(20));             /* d (dS/l) / d a2 */
+    const T h = std::fma(a2, std::fma(a2, T(0.375), T(0.5)), T(1));   /* d dS / d l at fixed curvature */
+    const T gp = std::fma(a2, T(3) / T(20), c16);                     /* d (dS/l) / d a2 */
     J[1][2] = (tsm * J[0][2]) * h;
     J[1][3] = dS;
-    J[1][4] = (tsm * J[0][4]) * h + t * (((a * gp) * CB) * (l * l));
-    /* C2 = J C J^T: lower triangle, sums in ascending index order, then mirrored (no process noise) */
+    J[1][4] = std::fma(tsm * J[0][4], h, t * (((a * gp) * CB) * (l * l)));
+    /* C2 = J C J^T: lower triangle, fused multiply-adds in ascending index order, then mirrored (no process noise) */
     T A[5][5];
     for (int i = 0; i < 5; i++)
         for (int j = 0; j < 5; j++) {
             T acc = T(0);
-            for (int m = 0; m < 5; m++) acc = acc + J[i][m] * st.C[m][j];
+            for (int m = 0; m < 5; m++) acc = std::fma(J[i][m], st.C[m][j], acc);
             A[i][j] = acc;
         }
     T C2[5][5];
     for (int i = 0; i < 5; i++)
         for (int j = 0; j <= i; j++) {
             T acc = T(0);
-            for (int m = 0; m < 5; m++) acc = acc + A[i][m] * J[j][m];
+            for (int m = 0; m < 5; m++) acc = std::fma(A[i][m], J[j][m], acc);
             C2[i][j] = acc;
             C2[j][i] = acc;
         }
-    st.p[0] = y + dy;
-    st.p[1] = z + t * dS;
+    st.p[0] = std::fma(dx, tg, y);
+    st.p[1] = std::fma(t, dS, z);
     st.p[2] = s2;
     st.x = x2;
     std::memcpy(st.C, C2, sizeof(C2));
@@ -120,14 +120,14 @@ template <class T> void update1(State<T> &st, int i, T m, T e2) {
     const T w = T(1) / S;
     T K[5], row[5];
     for (int a = 0; a < 5; a++) { K[a] = st.C[a][i] * w; row[a] = st.C[i][a]; }
-    for (int a = 0; a < 5; a++) st.p[a] = st.p[a] + K[a] * r;
+    for (int a = 0; a < 5; a++) st.p[a] = std::fma(K[a], r, st.p[a]);
     for (int a = 0; a < 5; a++)
         for (int b = 0; b <= a; b++) {
-            const T v = st.C[a][b] - K[a] * row[b];
+            const T v = std::fma(-K[a], row[b], st.C[a][b]);
             st.C[a][b] = v;
             st.C[b][a] = v;
         }
-    st.chi2 = st.chi2 + (r * r) * w;
+    st.chi2 = std::fma(r * r, w, st.chi2);
 }
 
 /* A hit = two sequential scalar updates, y first, then z (uncorrelated errors). */

@@ -12,19 +12,35 @@ constexpr int kRowPad = 4;             // a row's sorted hits start at a multipl
 constexpr int kMaxBinsPerRow = 8192;   // K1 histogram lives in shared memory (32 KB)
 constexpr float kGridMargin = 1e-3f;   // [cm] slack of every bin-range query; the exact window test follows
 
-// One (sector,row).  Host fills the first 8 words when an event is finalised; K1 fills the grid.
-struct __align__(16) RowInfo {
+// One (sector,row), hot part: exactly the eight words a grid query needs (two 16-byte loads, no dead lanes:
+// a partly-used vector load makes the unused destination registers a write-after-write hazard for whatever the
+// compiler puts there next, which serialises the "prefetched" load).  Host fills hitOff/binOff; K1 fills the grid.
+struct __align__(32) RowGrid {
     int32_t hitOff;    // offset of the row's sorted hits in hits[]/orig[]/links/weight (multiple of kRowPad)
-    int32_t n;         // clusters in the row
-    int32_t inOff;     // offset of the row's clusters in the staging arrays, as loaded
-    int32_t binOff;    // offset of the row's binStart[nBins+1]
-    uint32_t gidBase;  // event-global id of load index 0 (canonical ids; DESIGN.md "ids")
-    int32_t maxBins;   // capacity reserved for this row's bins
-    int32_t nY, nZ;    // grid dimensions (K1)
+    int32_t binOff;    // offset of the row's binStart[nBins+1] / buckets[nBins]
+    int32_t nY, nZ;    // grid dimensions (K1; 1x1 with an empty bucket for an empty row)
     float y0, z0;      // grid origin (K1)
     float invY, invZ;  // 1 / bin size (K1)
 };
-static_assert(sizeof(RowInfo) == 48, "RowInfo layout");
+static_assert(sizeof(RowGrid) == 32, "RowGrid layout");
+
+// One (sector,row), cold part (host-filled).
+struct __align__(16) RowMeta {
+    int32_t n;         // clusters in the row
+    int32_t inOff;     // offset of the row's clusters in the staging arrays, as loaded
+    uint32_t gidBase;  // event-global id of load index 0 (canonical ids; DESIGN.md "ids")
+    int32_t maxBins;   // capacity reserved for this row's bins
+};
+static_assert(sizeof(RowMeta) == 16, "RowMeta layout");
+
+// One grid bin, one 32-byte sector: where the bin's hits start in the sorted arrays, how many there are, and the
+// first three of them inline, so that a road search costs ONE dependent memory level instead of two
+// (binStart -> hits).  Bins with more than three hits continue in hits[start+3 ...].
+struct __align__(32) Bucket {
+    uint32_t start, count;
+    float2 h[3];
+};
+static_assert(sizeof(Bucket) == 32, "Bucket layout");
 
 // Per-tracklet record written by K5 (128 B, float4-aligned).
 struct __align__(16) TrackletRec {
@@ -43,17 +59,19 @@ struct DevParams {
     int32_t nSec, nRows;
 };
 
-enum Counter { kNStart = 0, kQueue = 1, kNTracks = 2, kNTrackClusters = 3, kNKept = 4, kHitsTotal = 5, kNLinks = 6, kNCounters = 16 };
+enum Counter { kNStart = 0, kQueue = 1, kQueue2 = 7, kNTracks = 2, kNTrackClusters = 3, kNKept = 4, kHitsTotal = 5, kNLinks = 6, kNCounters = 16 };
 
 // All device pointers of one tracker; passed by value to the kernels.
 struct DevPtrs {
     const float* inY;
     const float* inZ;
-    RowInfo* rows;
+    RowGrid* grid;         // [nRowsTotal]
+    const RowMeta* meta;   // [nRowsTotal]
     const float* rowX;
     float2* hits;          // sorted (y,z) pairs
     uint32_t* orig;        // sorted position -> load index
     uint32_t* binStart;
+    Bucket* buckets;       // [binCap], same indexing as binStart (row.binOff + bin)
     int32_t* linkUp;       // raw links, index = sorted position in the adjacent row
     int32_t* linkDn;
     int32_t* linkUpC;      // cleaned links

@@ -23,16 +23,26 @@ __global__ void __launch_bounds__(kK1Threads) k1_sort_grid(DevPtrs d) {
     const int rowId = blockIdx.x;
     const int tid = threadIdx.x;
     if (rowId == 0 && tid < kNCounters) d.counters[tid] = 0u;
-    RowInfo R = d.rows[rowId];
-    const int n = R.n;
-    if (n == 0) return;
+    const RowMeta M = d.meta[rowId];
+    RowGrid R = d.grid[rowId];
+    const int n = M.n;
+    if (n == 0) {   // empty row: the host's default 1x1 grid stays; give it an empty bucket
+        if (tid == 0) {
+            const float qn = __int_as_float(0x7fc00000);
+            float4* q = reinterpret_cast<float4*>(d.buckets + R.binOff);
+            q[0] = make_float4(0.f, 0.f, qn, qn);
+            q[1] = make_float4(qn, qn, qn, qn);
+            d.binStart[R.binOff] = 0u; d.binStart[R.binOff + 1] = 0u;
+        }
+        return;
+    }
     extern __shared__ uint32_t sh[];            // [maxBins + 1] histogram / cursors
     __shared__ float redA[4][kK1Threads / 32];
     __shared__ uint32_t warpSum[kK1Threads / 32];
     __shared__ int sNY, sNZ;
     __shared__ float sY0, sZ0, sInvY, sInvZ;
-    const float* __restrict__ y = d.inY + R.inOff;
-    const float* __restrict__ z = d.inZ + R.inOff;
+    const float* __restrict__ y = d.inY + M.inOff;
+    const float* __restrict__ z = d.inZ + M.inOff;
 
     // 1. bounding box
     float ymin = 3.0e38f, ymax = -3.0e38f, zmin = 3.0e38f, zmax = -3.0e38f;
@@ -60,7 +70,7 @@ __global__ void __launch_bounds__(kK1Threads) k1_sort_grid(DevPtrs d) {
         zmin = fminf(fmaxf(zmin, -1.0e4f), 1.0e4f); zmax = fminf(fmaxf(zmax, -1.0e4f), 1.0e4f);
         const float spanY = fmaxf(ymax - ymin, 1.0e-2f), spanZ = fmaxf(zmax - zmin, 1.0e-2f);
         // about one hit per bin, bins twice as long in z as in y (a query costs per z-bin-row), >= 0.5 cm
-        const int target = max(1, min(R.maxBins, n));
+        const int target = max(1, min(M.maxBins, n));
         float ey = sqrtf(spanY * spanZ / (2.0f * (float)target));
         ey = fmaxf(ey, 0.5f);
         int nY = max(1, min(target, (int)(spanY / ey)));
@@ -68,7 +78,7 @@ __global__ void __launch_bounds__(kK1Threads) k1_sort_grid(DevPtrs d) {
         sNY = nY; sNZ = nZ; sY0 = ymin; sZ0 = zmin;
         sInvY = (float)nY / spanY; sInvZ = (float)nZ / spanZ;
         R.nY = nY; R.nZ = nZ; R.y0 = ymin; R.z0 = zmin; R.invY = sInvY; R.invZ = sInvZ;
-        d.rows[rowId] = R;
+        d.grid[rowId] = R;
     }
     __syncthreads();
     const int nY = sNY, nZ = sNZ, nBins = nY * nZ;
@@ -119,11 +129,26 @@ __global__ void __launch_bounds__(kK1Threads) k1_sort_grid(DevPtrs d) {
         og[pos] = (uint32_t)i;
         wt[i] = 0u;
     }
+    __syncthreads();
+
+    // 5. buckets: after the scatter sh[b] is the END of bin b, so bin b starts at sh[b-1]
+    Bucket* __restrict__ bk = d.buckets + R.binOff;
+    const float qnan = __int_as_float(0x7fc00000);
+    for (int b = tid; b < nBins; b += kK1Threads) {
+        const uint32_t s0 = b ? sh[b - 1] : 0u, cnt = sh[b] - s0;
+        float2 h0 = make_float2(qnan, qnan), h1 = h0, h2 = h0;   // NaN never passes a window test
+        if (cnt > 0) h0 = hs[s0];
+        if (cnt > 1) h1 = hs[s0 + 1];
+        if (cnt > 2) h2 = hs[s0 + 2];
+        float4* q = reinterpret_cast<float4*>(bk + b);
+        q[0] = make_float4(__uint_as_float(s0), __uint_as_float(cnt), h0.x, h0.y);
+        q[1] = make_float4(h1.x, h1.y, h2.x, h2.y);
+    }
 }
 
 // Enumerate every hit of row R whose bin overlaps [yc-wy, yc+wy] x [zc-wz, zc+wz] (a superset of the window).
 template <class F>
-__device__ __forceinline__ void for_window(const RowInfo& R, const float2* __restrict__ hits,
+__device__ __forceinline__ void for_window(const RowGrid& R, const float2* __restrict__ hits,
                                            const uint32_t* __restrict__ binStart, float yc, float zc, float wy,
                                            float wz, F&& f) {
     const int by0 = bin_of(yc - wy - kGridMargin, R.y0, R.invY, R.nY);
@@ -146,18 +171,19 @@ constexpr int kK2Cap = 16;   // down-candidates cached per thread; beyond that a
 __global__ void __launch_bounds__(kK2Threads) k2_neighbours(DevPtrs d, DevParams dp) {
     const int rowId = blockIdx.x;
     const int r = rowId % dp.nRows;
-    const RowInfo R = d.rows[rowId];
-    if (R.n == 0) return;
+    const int n = d.meta[rowId].n;
+    if (n == 0) return;
+    const RowGrid R = d.grid[rowId];
     int32_t* __restrict__ up = d.linkUp + R.hitOff;
     int32_t* __restrict__ dn = d.linkDn + R.hitOff;
     bool active = (r >= 1 && r <= dp.nRows - 2);
-    RowInfo Ru, Rd;
+    RowGrid Ru = R, Rd = R;
     if (active) {
-        Ru = d.rows[rowId + 1]; Rd = d.rows[rowId - 1];
-        active = Ru.n > 0 && Rd.n > 0;
+        Ru = d.grid[rowId + 1]; Rd = d.grid[rowId - 1];
+        active = d.meta[rowId + 1].n > 0 && d.meta[rowId - 1].n > 0;
     }
     if (!active) {
-        for (int i = threadIdx.x; i < R.n; i += kK2Threads) { up[i] = -1; dn[i] = -1; }
+        for (int i = threadIdx.x; i < n; i += kK2Threads) { up[i] = -1; dn[i] = -1; }
         return;
     }
     const float xr = d.rowX[r];
@@ -169,7 +195,7 @@ __global__ void __launch_bounds__(kK2Threads) k2_neighbours(DevPtrs d, DevParams
     const uint32_t* __restrict__ origU = d.orig + Ru.hitOff;
     const uint32_t* __restrict__ origD = d.orig + Rd.hitOff;
 
-    for (int i = threadIdx.x; i < R.n; i += kK2Threads) {
+    for (int i = threadIdx.x; i < n; i += kK2Threads) {
         const float2 h = d.hits[R.hitOff + i];
         float cy[kK2Cap], cz[kK2Cap];
         int ck[kK2Cap];
@@ -220,36 +246,36 @@ __global__ void __launch_bounds__(kK2Threads) k2_neighbours(DevPtrs d, DevParams
 // kernel does both; the start list is appended with one atomic per warp (ballot + prefix).
 constexpr int kK3Threads = 128;
 
-__device__ __forceinline__ int clean_up_link(const DevPtrs& d, const RowInfo& R, const RowInfo& Rup, int i) {
-    const int u = d.linkUp[R.hitOff + i];
-    return (u >= 0 && d.linkDn[Rup.hitOff + u] == i) ? u : -1;
+__device__ __forceinline__ int clean_up_link(const DevPtrs& d, int hitOff, int hitOffUp, int i) {
+    const int u = d.linkUp[hitOff + i];
+    return (u >= 0 && d.linkDn[hitOffUp + u] == i) ? u : -1;
 }
 
 __global__ void __launch_bounds__(kK3Threads) k3_clean_start(DevPtrs d, DevParams dp) {
     const int rowId = blockIdx.x;
     const int r = rowId % dp.nRows;
-    const RowInfo R = d.rows[rowId];
-    if (R.n == 0) return;
+    const int n = d.meta[rowId].n;
+    if (n == 0) return;
     const bool hasUp = r + 1 < dp.nRows, hasDn = r >= 1;
-    RowInfo Ru = R, Rd = R;
-    if (hasUp) Ru = d.rows[rowId + 1];
-    if (hasDn) Rd = d.rows[rowId - 1];
+    const int hitOff = d.grid[rowId].hitOff;
+    const int hitOffU = hasUp ? d.grid[rowId + 1].hitOff : hitOff;
+    const int hitOffD = hasDn ? d.grid[rowId - 1].hitOff : hitOff;
     const unsigned lane = threadIdx.x & 31u;
     unsigned nLinks = 0;
-    for (int base = 0; base < R.n; base += kK3Threads) {
+    for (int base = 0; base < n; base += kK3Threads) {
         const int i = base + threadIdx.x;
         bool isStart = false;
-        if (i < R.n) {
-            const int u = d.linkUp[R.hitOff + i], dnl = d.linkDn[R.hitOff + i];
-            const int uc = (u >= 0 && d.linkDn[Ru.hitOff + u] == i) ? u : -1;
-            const int dc = (dnl >= 0 && d.linkUp[Rd.hitOff + dnl] == i) ? dnl : -1;
-            d.linkUpC[R.hitOff + i] = uc;
-            d.linkDnC[R.hitOff + i] = dc;
+        if (i < n) {
+            const int u = d.linkUp[hitOff + i], dnl = d.linkDn[hitOff + i];
+            const int uc = (u >= 0 && d.linkDn[hitOffU + u] == i) ? u : -1;
+            const int dc = (dnl >= 0 && d.linkUp[hitOffD + dnl] == i) ? dnl : -1;
+            d.linkUpC[hitOff + i] = uc;
+            d.linkDnC[hitOff + i] = dc;
             nLinks += uc >= 0;
             if (dc < 0 && uc >= 0) {
                 int len = 2, cur = uc, row = rowId + 1;
                 while (len < dp.P.seed_min_chain && (row % dp.nRows) + 1 < dp.nRows) {
-                    const int nx = clean_up_link(d, d.rows[row], d.rows[row + 1], cur);
+                    const int nx = clean_up_link(d, d.grid[row].hitOff, d.grid[row + 1].hitOff, cur);
                     if (nx < 0) break;
                     cur = nx; row++; len++;
                 }

@@ -21,7 +21,7 @@ constexpr size_t kAlign = 256;
 inline size_t align_up(size_t v, size_t a = kAlign) { return (v + a - 1) / a * a; }
 
 struct Layout {   // byte offsets into the workspace
-    size_t inY, inZ, rows, rowX, hits, orig, binStart, linkUp, linkDn, linkUpC, linkDnC, weight, starts, recs, rowHit,
+    size_t inY, inZ, grid, meta, rowX, hits, orig, binStart, buckets, linkUp, linkDn, linkUpC, linkDnC, weight, starts, recs, rowHit,
         tracks, clusterIds, counters, sectorGidBase, total;
     int64_t hitCap, binCap, maxTracklets;
 };
@@ -51,7 +51,8 @@ struct tpc_tracker {
     float* hostY = nullptr; float* hostZ = nullptr; int64_t hostCap = 0;   // pinned mirror for host-pointer loads
     int64_t dirtyLo = 0, dirtyHi = 0;       // host-staged range not yet uploaded
     cudaEvent_t evUpload = nullptr; bool uploadPending = false;
-    RowInfo* hostRows = nullptr;            // pinned
+    RowGrid* hostGrid = nullptr;            // pinned
+    RowMeta* hostMeta = nullptr;            // pinned
     uint32_t* hostSectorBase = nullptr;     // pinned
     uint32_t* hostCounters = nullptr;       // pinned
     int maxBinsLaunch = 1;
@@ -84,11 +85,13 @@ Layout make_layout(const tpc_tracker* t, int64_t maxClusters) {
     auto take = [&](size_t bytes) { size_t r = o; o = align_up(o + bytes); return r; };
     L.inY = take(sizeof(float) * (maxClusters + 16));
     L.inZ = take(sizeof(float) * (maxClusters + 16));
-    L.rows = take(sizeof(RowInfo) * (NR + 2));
+    L.grid = take(sizeof(RowGrid) * (NR + 2));
+    L.meta = take(sizeof(RowMeta) * (NR + 2));
     L.rowX = take(sizeof(float) * (t->nRows + 1));
     L.hits = take(sizeof(float2) * L.hitCap);
     L.orig = take(sizeof(uint32_t) * L.hitCap);
     L.binStart = take(sizeof(uint32_t) * L.binCap);
+    L.buckets = take(sizeof(Bucket) * L.binCap);
     L.linkUp = take(sizeof(int32_t) * L.hitCap);
     L.linkDn = take(sizeof(int32_t) * L.hitCap);
     L.linkUpC = take(sizeof(int32_t) * L.hitCap);
@@ -110,8 +113,8 @@ void bind_pointers(tpc_tracker* t) {
     const Layout& L = t->L;
     DevPtrs& d = t->dev;
     d.inY = (const float*)(w + L.inY); d.inZ = (const float*)(w + L.inZ);
-    d.rows = (RowInfo*)(w + L.rows); d.rowX = (const float*)(w + L.rowX);
-    d.hits = (float2*)(w + L.hits); d.orig = (uint32_t*)(w + L.orig); d.binStart = (uint32_t*)(w + L.binStart);
+    d.grid = (RowGrid*)(w + L.grid); d.meta = (const RowMeta*)(w + L.meta); d.rowX = (const float*)(w + L.rowX);
+    d.hits = (float2*)(w + L.hits); d.orig = (uint32_t*)(w + L.orig); d.binStart = (uint32_t*)(w + L.binStart); d.buckets = (Bucket*)(w + L.buckets);
     d.linkUp = (int32_t*)(w + L.linkUp); d.linkDn = (int32_t*)(w + L.linkDn);
     d.linkUpC = (int32_t*)(w + L.linkUpC); d.linkDnC = (int32_t*)(w + L.linkDnC);
     d.weight = (uint32_t*)(w + L.weight); d.starts = (int2*)(w + L.starts);
@@ -164,30 +167,29 @@ int flush_dirty(tpc_tracker* t) {
 int finalize_event(tpc_tracker* t) {
     if (t->finalized) return TPC_OK;
     const int NR = t->nRowsTotal;
-    if (!t->hostRows) {
-        CUDA_TRY(t, cudaMallocHost(&t->hostRows, sizeof(RowInfo) * (NR + 2)));
+    if (!t->hostGrid) {
+        CUDA_TRY(t, cudaMallocHost(&t->hostGrid, sizeof(RowGrid) * (NR + 2)));
+        CUDA_TRY(t, cudaMallocHost(&t->hostMeta, sizeof(RowMeta) * (NR + 2)));
         CUDA_TRY(t, cudaMallocHost(&t->hostSectorBase, sizeof(uint32_t) * (t->nSec + 1)));
         CUDA_TRY(t, cudaMallocHost(&t->hostCounters, sizeof(uint32_t) * kNCounters));
     } else {
-        CUDA_TRY(t, cudaStreamSynchronize(t->stream));   // a previous async upload may still read hostRows
+        CUDA_TRY(t, cudaStreamSynchronize(t->stream));   // a previous async upload may still read the host tables
     }
     int64_t gid = 0, hitOff = 0, binOff = 0;
     int maxBins = 1;
     for (int i = 0; i < NR; i++) {
-        RowInfo& R = t->hostRows[i];
-        std::memset(&R, 0, sizeof(R));
-        if (i % t->nRows == 0) {
-            t->hostSectorBase[i / t->nRows] = (uint32_t)gid;
-        }
+        RowGrid& G = t->hostGrid[i];
+        RowMeta& M = t->hostMeta[i];
+        if (i % t->nRows == 0) t->hostSectorBase[i / t->nRows] = (uint32_t)gid;
         const int n = t->rowN[i];
-        R.hitOff = (int32_t)hitOff; R.n = n; R.inOff = t->rowIn[i]; R.binOff = (int32_t)binOff;
-        R.gidBase = (uint32_t)gid;
-        R.maxBins = std::max(1, std::min(n, kMaxBinsPerRow));
-        R.nY = R.nZ = 1; R.invY = R.invZ = 1.f;
-        maxBins = std::max(maxBins, R.maxBins);
+        G.hitOff = (int32_t)hitOff; G.binOff = (int32_t)binOff;
+        G.nY = G.nZ = 1; G.y0 = G.z0 = 0.f; G.invY = G.invZ = 1.f;
+        M.n = n; M.inOff = t->rowIn[i]; M.gidBase = (uint32_t)gid;
+        M.maxBins = std::max(1, std::min(n, kMaxBinsPerRow));
+        maxBins = std::max(maxBins, M.maxBins);
         gid += n;
         hitOff += (n + kRowPad - 1) / kRowPad * kRowPad;
-        binOff += R.maxBins + 1;
+        binOff += M.maxBins + 1;
     }
     t->hostSectorBase[t->nSec] = (uint32_t)gid;
     for (int s = 0; s < t->nSec; s++)
@@ -195,7 +197,8 @@ int finalize_event(tpc_tracker* t) {
     t->nClusters = gid;
     t->maxBinsLaunch = maxBins;
     if (gid > t->maxClusters || hitOff > t->L.hitCap || binOff > t->L.binCap) return TPC_E_NOMEM;
-    CUDA_TRY(t, cudaMemcpyAsync(t->dev.rows, t->hostRows, sizeof(RowInfo) * NR, cudaMemcpyHostToDevice, t->stream));
+    CUDA_TRY(t, cudaMemcpyAsync(t->dev.grid, t->hostGrid, sizeof(RowGrid) * NR, cudaMemcpyHostToDevice, t->stream));
+    CUDA_TRY(t, cudaMemcpyAsync((void*)t->dev.meta, t->hostMeta, sizeof(RowMeta) * NR, cudaMemcpyHostToDevice, t->stream));
     CUDA_TRY(t, cudaMemcpyAsync(t->dev.sectorGidBase, t->hostSectorBase, sizeof(uint32_t) * (t->nSec + 1),
                                 cudaMemcpyHostToDevice, t->stream));
     {
@@ -235,16 +238,17 @@ int stage_clusters(tpc_tracker* t, int64_t at, int64_t n, const float* y, const 
 // ---- debug-dump conversion kernels (tests only; not on the hot path)
 __global__ void dump_links_kernel(DevPtrs d, int nRows, int64_t N, int32_t* out) {
     const int rowId = blockIdx.x, r = rowId % nRows;
-    const RowInfo R = d.rows[rowId];
-    for (int k = threadIdx.x; k < R.n; k += blockDim.x) {
-        const int64_t g = (int64_t)R.gidBase + d.orig[R.hitOff + k];
+    const RowGrid R = d.grid[rowId];
+    const RowMeta M = d.meta[rowId];
+    for (int k = threadIdx.x; k < M.n; k += blockDim.x) {
+        const int64_t g = (int64_t)M.gidBase + d.orig[R.hitOff + k];
         const int32_t* src[4] = {d.linkUp, d.linkDn, d.linkUpC, d.linkDnC};
         for (int w = 0; w < 4; w++) {
             const int l = src[w][R.hitOff + k];
             int v = -1;
             if (l >= 0) {
                 const bool upw = (w % 2) == 0;
-                if ((upw && r + 1 < nRows) || (!upw && r >= 1)) v = (int)d.orig[d.rows[rowId + (upw ? 1 : -1)].hitOff + l];
+                if ((upw && r + 1 < nRows) || (!upw && r >= 1)) v = (int)d.orig[d.grid[rowId + (upw ? 1 : -1)].hitOff + l];
             }
             out[(int64_t)w * N + g] = v;
         }
@@ -254,8 +258,7 @@ __global__ void dump_starts_kernel(DevPtrs d, unsigned n, uint32_t* out) {
     const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const int2 s = d.starts[i];
-    const RowInfo R = d.rows[s.x];
-    out[i] = R.gidBase + d.orig[R.hitOff + s.y];
+    out[i] = d.meta[s.x].gidBase + d.orig[d.grid[s.x].hitOff + s.y];
 }
 __global__ void dump_rowhit_kernel(DevPtrs d, int nRows, unsigned n, int32_t* out) {
     const unsigned slot = blockIdx.x;
@@ -265,18 +268,19 @@ __global__ void dump_rowhit_kernel(DevPtrs d, int nRows, unsigned n, int32_t* ou
         int v = -1;
         if (r >= t.firstRow && r <= t.lastRow) {
             const int h = d.rowHit[(size_t)slot * d.rhStride + r];
-            if (h >= 0) v = (int)d.orig[d.rows[t.sector * nRows + r].hitOff + h];
+            if (h >= 0) v = (int)d.orig[d.grid[t.sector * nRows + r].hitOff + h];
         }
         out[(size_t)slot * nRows + r] = v;
     }
 }
 __global__ void dump_owner_kernel(DevPtrs d, int nRows, uint32_t* out) {
     const int rowId = blockIdx.x;
-    const RowInfo R = d.rows[rowId];
+    const RowGrid R = d.grid[rowId];
+    const RowMeta M = d.meta[rowId];
     const uint32_t sb = d.sectorGidBase[rowId / nRows];
-    for (int k = threadIdx.x; k < R.n; k += blockDim.x) {
+    for (int k = threadIdx.x; k < M.n; k += blockDim.x) {
         const uint32_t w = d.weight[R.hitOff + k];
-        out[R.gidBase + d.orig[R.hitOff + k]] = w ? sb + (0x00FFFFFFu - (w & 0x00FFFFFFu)) : 0xFFFFFFFFu;
+        out[M.gidBase + d.orig[R.hitOff + k]] = w ? sb + (0x00FFFFFFu - (w & 0x00FFFFFFu)) : 0xFFFFFFFFu;
     }
 }
 
@@ -321,7 +325,8 @@ void tpc_tracker_destroy(tpc_tracker* t) {
     if (t->stream || t->ws) cudaStreamSynchronize(t->stream);
     if (t->hostY) cudaFreeHost(t->hostY);
     if (t->hostZ) cudaFreeHost(t->hostZ);
-    if (t->hostRows) cudaFreeHost(t->hostRows);
+    if (t->hostGrid) cudaFreeHost(t->hostGrid);
+    if (t->hostMeta) cudaFreeHost(t->hostMeta);
     if (t->hostSectorBase) cudaFreeHost(t->hostSectorBase);
     if (t->hostCounters) cudaFreeHost(t->hostCounters);
     if (t->outTracks) cudaFreeHost(t->outTracks);
@@ -364,7 +369,7 @@ int tpc_set_workspace(tpc_tracker* t, void* dev_ptr, size_t bytes) {
         int dev = 0, sms = 0, occ5 = 0, occ6 = 0;
         CUDA_TRY(t, cudaGetDevice(&dev));
         CUDA_TRY(t, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-        CUDA_TRY(t, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ5, k5_construct, kK5Threads, 0));
+        CUDA_TRY(t, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ5, k5_follow, kK5Threads, 0));
         CUDA_TRY(t, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ6, k6_select, kK6Threads, 0));
         t->k5Blocks = sms * std::max(1, occ5);
         t->k6Blocks = sms * std::max(1, occ6);
@@ -431,7 +436,8 @@ int tpc_track_sectors(tpc_tracker* t) {
     CUDA_TRY(t, cudaEventRecord(t->ev[2], s));
     k3_clean_start<<<NR, kK3Threads, 0, s>>>(d, dp);
     CUDA_TRY(t, cudaEventRecord(t->ev[3], s));
-    k5_construct<<<t->k5Blocks, kK5Threads, 0, s>>>(d, dp);
+    k5_follow<<<t->k5Blocks, kK5Threads, 0, s>>>(d, dp);
+    k5_refit<<<t->k5Blocks, kK5Threads, 0, s>>>(d, dp);
     CUDA_TRY(t, cudaEventRecord(t->ev[4], s));
     k6_weights<<<t->k6Blocks, kK6Threads, 0, s>>>(d, dp);
     CUDA_TRY(t, cudaEventRecord(t->ev[5], s));
@@ -442,7 +448,7 @@ int tpc_track_sectors(tpc_tracker* t) {
     return TPC_OK;
 }
 
-int tpc_launches_per_track(const tpc_tracker* t) { (void)t; return 6; }
+int tpc_launches_per_track(const tpc_tracker* t) { (void)t; return 7; }
 
 int tpc_sync(tpc_tracker* t) {
     if (!t) return TPC_E_ARG;
