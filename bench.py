@@ -205,6 +205,7 @@ def main():
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--bins-per-hit", type=float, default=None, help="override tpc_params.grid_bins_per_hit (tuning)")
     args = ap.parse_args()
     rank, world, local, dist = init_dist(args.gpus)
     if args.impl == "reference":
@@ -224,7 +225,10 @@ def main():
     warmup = max(args.warmup, 3)
 
     ev = datagen.config_event(args.config, seed=rank)
-    trk = binding.Tracker(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz)
+    params = binding.default_params()
+    if args.bins_per_hit is not None:
+        params.grid_bins_per_hit = args.bins_per_hit
+    trk = binding.Tracker(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz, params)
     stream = torch.cuda.current_stream()
     trk.set_stream(stream.cuda_stream)
     ws_bytes = trk.allocate_workspace(ev.n_clusters, device=dev)
@@ -313,7 +317,8 @@ def main():
                    "n_clusters_total": n_total, "events_per_sec": world / (ms * 1e-3), "seed": "rank", "l2": "flushed (256 MiB write) before every timed step",
                    "parallelism": "one event per GPU, no collective" if world > 1 else "single GPU",
                    "n_start_hits": st["n_start_hits"], "n_tracklet_hits": st["n_tracklet_hits"], "n_tracks": st["n_tracks"],
-                   "workspace_bytes": ws_bytes, "workspace_over_input": round(ws_bytes / (12.0 * ev.n_clusters), 2)},
+                   "workspace_bytes": ws_bytes, "workspace_over_input": round(ws_bytes / (12.0 * ev.n_clusters), 2),
+                   "grid_bins_per_hit": float(params.grid_bins_per_hit)},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms_max, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
         "gpu_launches": args.steps * trk.launches_per_track(),

@@ -22,7 +22,7 @@ class tpc_params(ctypes.Structure):
         ("kf_ctt0", ctypes.c_float), ("kf_ckk0", ctypes.c_float), ("kf_smax", ctypes.c_float),
         ("road_nsig", ctypes.c_float), ("road_max", ctypes.c_float), ("max_gap", ctypes.c_int32),
         ("min_hits", ctypes.c_int32), ("seed_min_chain", ctypes.c_int32),
-        ("max_tracklets_per_cluster", ctypes.c_float),
+        ("max_tracklets_per_cluster", ctypes.c_float), ("grid_bins_per_hit", ctypes.c_float),
     ]
 
 

@@ -59,7 +59,7 @@ struct DevParams {
     int32_t nSec, nRows;
 };
 
-enum Counter { kNStart = 0, kQueue = 1, kQueue2 = 7, kNTracks = 2, kNTrackClusters = 3, kNKept = 4, kHitsTotal = 5, kNLinks = 6, kNCounters = 16 };
+enum Counter { kNStart = 0, kQueue = 1, kNTracks = 2, kNTrackClusters = 3, kNKept = 4, kHitsTotal = 5, kNLinks = 6, kNCounters = 16 };
 
 // All device pointers of one tracker; passed by value to the kernels.
 struct DevPtrs {

@@ -69,8 +69,8 @@ __global__ void __launch_bounds__(kK1Threads) k1_sort_grid(DevPtrs d) {
         ymin = fminf(fmaxf(ymin, -1.0e4f), 1.0e4f); ymax = fminf(fmaxf(ymax, -1.0e4f), 1.0e4f);
         zmin = fminf(fmaxf(zmin, -1.0e4f), 1.0e4f); zmax = fminf(fmaxf(zmax, -1.0e4f), 1.0e4f);
         const float spanY = fmaxf(ymax - ymin, 1.0e-2f), spanZ = fmaxf(zmax - zmin, 1.0e-2f);
-        // about one hit per bin, bins twice as long in z as in y (a query costs per z-bin-row), >= 0.5 cm
-        const int target = max(1, min(M.maxBins, n));
+        // kBinsPerHit bins per hit, bins twice as long in z as in y (a query costs per z-bin-row), >= 0.5 cm
+        const int target = max(1, M.maxBins);
         float ey = sqrtf(spanY * spanZ / (2.0f * (float)target));
         ey = fmaxf(ey, 0.5f);
         int nY = max(1, min(target, (int)(spanY / ey)));

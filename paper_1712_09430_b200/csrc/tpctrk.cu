@@ -79,7 +79,7 @@ Layout make_layout(const tpc_tracker* t, int64_t maxClusters) {
     Layout L{};
     const int64_t NR = t->nRowsTotal;
     L.hitCap = maxClusters + (int64_t)kRowPad * NR + 16;
-    L.binCap = maxClusters + 2 * NR + 16;
+    L.binCap = (int64_t)((double)maxClusters * (double)t->P.grid_bins_per_hit) + 2 * NR + 16;
     L.maxTracklets = (int64_t)((double)maxClusters * (double)t->P.max_tracklets_per_cluster) + 4096;
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t r = o; o = align_up(o + bytes); return r; };
@@ -185,7 +185,7 @@ int finalize_event(tpc_tracker* t) {
         G.hitOff = (int32_t)hitOff; G.binOff = (int32_t)binOff;
         G.nY = G.nZ = 1; G.y0 = G.z0 = 0.f; G.invY = G.invZ = 1.f;
         M.n = n; M.inOff = t->rowIn[i]; M.gidBase = (uint32_t)gid;
-        M.maxBins = std::max(1, std::min(n, kMaxBinsPerRow));
+        M.maxBins = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)((double)n * (double)t->P.grid_bins_per_hit), kMaxBinsPerRow));
         maxBins = std::max(maxBins, M.maxBins);
         gid += n;
         hitOff += (n + kRowPad - 1) / kRowPad * kRowPad;
@@ -296,6 +296,7 @@ void tpc_default_params(tpc_params* p) {
     p->road_nsig = 4.0f; p->road_max = 2.0f;
     p->max_gap = 4; p->min_hits = 10; p->seed_min_chain = 3;
     p->max_tracklets_per_cluster = 0.125f;
+    p->grid_bins_per_hit = 4.0f;
 }
 
 int tpc_tracker_create(const tpc_geometry* g, float bz_tesla, tpc_tracker** out) {
@@ -310,7 +311,8 @@ int tpc_tracker_create(const tpc_geometry* g, float bz_tesla, tpc_tracker** out)
     t->rhStride = (g->n_rows + 31) / 32 * 32;
     t->rowX.assign(g->row_x, g->row_x + g->n_rows);
     if (g->params) t->P = *g->params; else tpc_default_params(&t->P);
-    if (t->P.seed_min_chain < 2 || t->P.min_hits < 1 || t->P.max_gap < 0 || !(t->P.max_tracklets_per_cluster > 0.f)) {
+    if (t->P.seed_min_chain < 2 || t->P.min_hits < 1 || t->P.max_gap < 0 || !(t->P.max_tracklets_per_cluster > 0.f) ||
+        !(t->P.grid_bins_per_hit >= 0.25f && t->P.grid_bins_per_hit <= 64.f)) {
         delete t; return TPC_E_ARG;
     }
     t->bz = bz_tesla;
@@ -369,7 +371,7 @@ int tpc_set_workspace(tpc_tracker* t, void* dev_ptr, size_t bytes) {
         int dev = 0, sms = 0, occ5 = 0, occ6 = 0;
         CUDA_TRY(t, cudaGetDevice(&dev));
         CUDA_TRY(t, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-        CUDA_TRY(t, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ5, k5_follow, kK5Threads, 0));
+        CUDA_TRY(t, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ5, k5_construct, kK5Threads, 0));
         CUDA_TRY(t, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ6, k6_select, kK6Threads, 0));
         t->k5Blocks = sms * std::max(1, occ5);
         t->k6Blocks = sms * std::max(1, occ6);
@@ -436,8 +438,7 @@ int tpc_track_sectors(tpc_tracker* t) {
     CUDA_TRY(t, cudaEventRecord(t->ev[2], s));
     k3_clean_start<<<NR, kK3Threads, 0, s>>>(d, dp);
     CUDA_TRY(t, cudaEventRecord(t->ev[3], s));
-    k5_follow<<<t->k5Blocks, kK5Threads, 0, s>>>(d, dp);
-    k5_refit<<<t->k5Blocks, kK5Threads, 0, s>>>(d, dp);
+    k5_construct<<<t->k5Blocks, kK5Threads, 0, s>>>(d, dp);
     CUDA_TRY(t, cudaEventRecord(t->ev[4], s));
     k6_weights<<<t->k6Blocks, kK6Threads, 0, s>>>(d, dp);
     CUDA_TRY(t, cudaEventRecord(t->ev[5], s));
@@ -448,7 +449,7 @@ int tpc_track_sectors(tpc_tracker* t) {
     return TPC_OK;
 }
 
-int tpc_launches_per_track(const tpc_tracker* t) { (void)t; return 7; }
+int tpc_launches_per_track(const tpc_tracker* t) { (void)t; return 6; }
 
 int tpc_sync(tpc_tracker* t) {
     if (!t) return TPC_E_ARG;

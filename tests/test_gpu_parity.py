@@ -213,3 +213,17 @@ def test_non_default_parameters():
     trk, tracks, ids = run_gpu(ev, pg)
     out = compare(ev, trk, tracks, ids, ref)
     assert out["tracklet_mismatch"] == 0
+
+
+@pytest.mark.parametrize("bph", [0.5, 1.0, 2.0, 16.0])
+def test_grid_resolution_does_not_change_any_result(bph):
+    """The y/z grid is an accelerator only (S1): coarse grids push the road search onto its exact
+    out-of-line path (bucket overflow), fine grids onto the multi-bin path; every stage must still match the oracle."""
+    _cuda()
+    ev = datagen.config_event(2, seed=3)
+    ref = oracle.run_event(ev)
+    p = binding.default_params()
+    p.grid_bins_per_hit = bph
+    trk, tracks, ids = run_gpu(ev, p)
+    out = compare(ev, trk, tracks, ids, ref)
+    assert out["tracklet_mismatch"] == 0 and out["link_mismatch_0"] == 0
