@@ -67,7 +67,9 @@ def lib():
     """Load libtpctrk.so (building it if sources are newer).  Raises if it cannot be built or loaded."""
     global _lib
     if _lib is None:
-        path = _build.build() if (_build.needs_build() and os.path.exists(_build.SOURCES[0])) else _build.LIB
+        path = os.environ.get("TPCTRK_LIB")   # an explicitly given build of the same library (tuning experiments)
+        if not path:
+            path = _build.build() if (_build.needs_build() and os.path.exists(_build.SOURCES[0])) else _build.LIB
         L = ctypes.CDLL(path)
         vp, i32, i64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64
         L.tpc_default_params.argtypes = [ctypes.POINTER(tpc_params)]

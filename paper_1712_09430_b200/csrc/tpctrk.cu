@@ -65,6 +65,7 @@ struct tpc_tracker {
     bool haveEvents = false;
     float kernelUs[8] = {0};
     int k5Blocks = 0, k6Blocks = 0;
+    size_t k5GridSmem = 0; bool k5SmemGrid = false;
 };
 
 namespace {
@@ -371,7 +372,15 @@ int tpc_set_workspace(tpc_tracker* t, void* dev_ptr, size_t bytes) {
         int dev = 0, sms = 0, occ5 = 0, occ6 = 0;
         CUDA_TRY(t, cudaGetDevice(&dev));
         CUDA_TRY(t, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-        CUDA_TRY(t, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ5, k5_construct, kK5Threads, 0));
+        // K5 keeps the whole row table in shared memory when it fits (one block per SM)
+        t->k5GridSmem = sizeof(RowGrid) * (size_t)t->nRowsTotal;
+        t->k5SmemGrid = t->k5GridSmem + 2048 <= 227 * 1024;
+        if (t->k5SmemGrid) {
+            CUDA_TRY(t, cudaFuncSetAttribute(k5_construct<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->k5GridSmem));
+            CUDA_TRY(t, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ5, k5_construct<true>, kK5Threads, t->k5GridSmem));
+        } else {
+            CUDA_TRY(t, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ5, k5_construct<false>, kK5Threads, 0));
+        }
         CUDA_TRY(t, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ6, k6_select, kK6Threads, 0));
         t->k5Blocks = sms * std::max(1, occ5);
         t->k6Blocks = sms * std::max(1, occ6);
@@ -438,7 +447,13 @@ int tpc_track_sectors(tpc_tracker* t) {
     CUDA_TRY(t, cudaEventRecord(t->ev[2], s));
     k3_clean_start<<<NR, kK3Threads, 0, s>>>(d, dp);
     CUDA_TRY(t, cudaEventRecord(t->ev[3], s));
-    k5_construct<<<t->k5Blocks, kK5Threads, 0, s>>>(d, dp);
+    {
+        // enough threads for the tracklet capacity, at most what is resident at once (persistent threads + queue)
+        const int64_t want = (t->L.maxTracklets + kK5Threads - 1) / kK5Threads;
+        const int blocks = (int)std::max<int64_t>(1, std::min<int64_t>(want, t->k5Blocks));
+        if (t->k5SmemGrid) k5_construct<true><<<blocks, kK5Threads, t->k5GridSmem, s>>>(d, dp);
+        else k5_construct<false><<<blocks, kK5Threads, 0, s>>>(d, dp);
+    }
     CUDA_TRY(t, cudaEventRecord(t->ev[4], s));
     k6_weights<<<t->k6Blocks, kK6Threads, 0, s>>>(d, dp);
     CUDA_TRY(t, cudaEventRecord(t->ev[5], s));
