@@ -77,7 +77,7 @@ struct DevPtrs {
     int32_t* linkUpC;      // cleaned links
     int32_t* linkDnC;
     uint32_t* weight;      // ownership key per hit
-    int2* starts;          // (rowId, sorted position)
+    int4* starts;          // (rowId, sorted position, sorted position of the linked hit in the row above, global id)
     TrackletRec* recs;
     int32_t* rowHit;       // [maxTracklets][rhStride], sorted position of the tracklet's hit in each row, -1 none
     tpc_track* tracks;

@@ -258,6 +258,7 @@ __global__ void __launch_bounds__(kK3Threads) k3_clean_start(DevPtrs d, DevParam
     if (n == 0) return;
     const bool hasUp = r + 1 < dp.nRows, hasDn = r >= 1;
     const int hitOff = d.grid[rowId].hitOff;
+    const uint32_t gidBase = d.meta[rowId].gidBase;
     const int hitOffU = hasUp ? d.grid[rowId + 1].hitOff : hitOff;
     const int hitOffD = hasDn ? d.grid[rowId - 1].hitOff : hitOff;
     const unsigned lane = threadIdx.x & 31u;
@@ -265,11 +266,13 @@ __global__ void __launch_bounds__(kK3Threads) k3_clean_start(DevPtrs d, DevParam
     for (int base = 0; base < n; base += kK3Threads) {
         const int i = base + threadIdx.x;
         bool isStart = false;
+        int upKeep = -1;
         if (i < n) {
             const int u = d.linkUp[hitOff + i], dnl = d.linkDn[hitOff + i];
             const int uc = (u >= 0 && d.linkDn[hitOffU + u] == i) ? u : -1;
             const int dc = (dnl >= 0 && d.linkUp[hitOffD + dnl] == i) ? dnl : -1;
             d.linkUpC[hitOff + i] = uc;
+            upKeep = uc;
             d.linkDnC[hitOff + i] = dc;
             nLinks += uc >= 0;
             if (dc < 0 && uc >= 0) {
@@ -287,7 +290,8 @@ __global__ void __launch_bounds__(kK3Threads) k3_clean_start(DevPtrs d, DevParam
             unsigned pos = 0;
             if (lane == 0) pos = atomicAdd(&d.counters[kNStart], (unsigned)__popc(m));
             pos = __shfl_sync(0xffffffffu, pos, 0) + __popc(m & ((1u << lane) - 1u));
-            if (isStart && pos < (unsigned)d.maxTracklets) d.starts[pos] = make_int2(rowId, i);
+            if (isStart && pos < (unsigned)d.maxTracklets)   // (row, hit, linked hit, canonical id): all K5 needs to begin
+                d.starts[pos] = make_int4(rowId, i, upKeep, (int)(gidBase + d.orig[hitOff + i]));
         }
     }
 #pragma unroll

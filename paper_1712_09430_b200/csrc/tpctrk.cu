@@ -98,7 +98,7 @@ Layout make_layout(const tpc_tracker* t, int64_t maxClusters) {
     L.linkUpC = take(sizeof(int32_t) * L.hitCap);
     L.linkDnC = take(sizeof(int32_t) * L.hitCap);
     L.weight = take(sizeof(uint32_t) * L.hitCap);
-    L.starts = take(sizeof(int2) * L.maxTracklets);
+    L.starts = take(sizeof(int4) * L.maxTracklets);
     L.recs = take(sizeof(TrackletRec) * L.maxTracklets);
     L.rowHit = take(sizeof(int32_t) * L.maxTracklets * t->rhStride);
     L.tracks = take(sizeof(tpc_track) * L.maxTracklets);
@@ -118,7 +118,7 @@ void bind_pointers(tpc_tracker* t) {
     d.hits = (float2*)(w + L.hits); d.orig = (uint32_t*)(w + L.orig); d.binStart = (uint32_t*)(w + L.binStart); d.buckets = (Bucket*)(w + L.buckets);
     d.linkUp = (int32_t*)(w + L.linkUp); d.linkDn = (int32_t*)(w + L.linkDn);
     d.linkUpC = (int32_t*)(w + L.linkUpC); d.linkDnC = (int32_t*)(w + L.linkDnC);
-    d.weight = (uint32_t*)(w + L.weight); d.starts = (int2*)(w + L.starts);
+    d.weight = (uint32_t*)(w + L.weight); d.starts = (int4*)(w + L.starts);
     d.recs = (TrackletRec*)(w + L.recs); d.rowHit = (int32_t*)(w + L.rowHit);
     d.tracks = (tpc_track*)(w + L.tracks); d.clusterIds = (uint32_t*)(w + L.clusterIds);
     d.counters = (uint32_t*)(w + L.counters); d.sectorGidBase = (uint32_t*)(w + L.sectorGidBase);
@@ -258,7 +258,7 @@ __global__ void dump_links_kernel(DevPtrs d, int nRows, int64_t N, int32_t* out)
 __global__ void dump_starts_kernel(DevPtrs d, unsigned n, uint32_t* out) {
     const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    const int2 s = d.starts[i];
+    const int4 s = d.starts[i];
     out[i] = d.meta[s.x].gidBase + d.orig[d.grid[s.x].hitOff + s.y];
 }
 __global__ void dump_rowhit_kernel(DevPtrs d, int nRows, unsigned n, int32_t* out) {
