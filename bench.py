@@ -37,7 +37,7 @@ def algorithmic_bytes(st: dict) -> dict:
     return {
         "K1_sort_grid": 8 * n + 8 * n + 4 * n + 4 * n + 4 * n,       # in y,z; out (y,z), orig, binStart(~N), weight=0
         "K2_neighbours": 8 * n + 4 * n + 8 * n,                      # hits once, bins once, links out
-        "K3K4_clean_start": 8 * n + 8 * n + 8 * s,                   # raw links in, cleaned out, start list
+        "K3K4_clean_start": 8 * n + 8 * n + 16 * s,                  # raw links in, cleaned out, start list (16 B each)
         "K5_construct": 28 * h + 4 * h + 128 * s,                    # per row step: link/bin 12 + hit 8 + cand 8; rowHit; record
         "K6a_weights": 4 * h + 8 * h + 32 * s,                       # rowHit in, atomicMax rmw, record header
         "K6b_select": 4 * h + 4 * h + 128 * s + 8 * c + 112 * t,     # rowHit, weight, record; orig + ids out, tracks out
