@@ -227,3 +227,29 @@ def test_grid_resolution_does_not_change_any_result(bph):
     trk, tracks, ids = run_gpu(ev, p)
     out = compare(ev, trk, tracks, ids, ref)
     assert out["tracklet_mismatch"] == 0 and out["link_mismatch_0"] == 0
+
+
+def test_geometry_whose_row_table_exceeds_shared_memory():
+    """K5 keeps the (sector,row) table in shared memory when it fits (36 x 159 rows: 183 KB); 40 x 200 rows need
+    256 KB and run the same kernel on the global table.  Straight tracks + noise, every stage against the oracle."""
+    _cuda()
+    n_sec, n_rows = 40, 200
+    rx = (85.0 + 0.8 * np.arange(n_rows)).astype(np.float32)
+    rng = np.random.default_rng(11)
+    hits = []
+    for _ in range(160):
+        s = int(rng.integers(0, n_sec))
+        a, b = rng.uniform(-8, 8), rng.uniform(-0.12, 0.12)
+        c, dz = rng.uniform(5, 120), rng.uniform(-0.4, 0.4)
+        r0, r1 = sorted(int(v) for v in rng.integers(0, n_rows, 2))
+        for r in range(r0, min(n_rows, r1 + 30)):
+            x = float(rx[r])
+            hits.append((s, r, a + b * (x - 85.0) + rng.normal(0, 0.1), c + dz * (x - 85.0) + rng.normal(0, 0.1)))
+    for _ in range(4000):
+        hits.append((int(rng.integers(0, n_sec)), int(rng.integers(0, n_rows)), rng.uniform(-15, 15), rng.uniform(0, 250)))
+    ev = datagen.event_from_hits(hits, n_sec, rx)
+    ref = oracle.run_event(ev)
+    assert ref.tracks.size > 50
+    trk, tracks, ids = run_gpu(ev)
+    out = compare(ev, trk, tracks, ids, ref)
+    assert out["tracklet_mismatch"] == 0 and out["link_mismatch_0"] == 0
