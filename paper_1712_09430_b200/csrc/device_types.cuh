@@ -69,7 +69,7 @@ struct DevPtrs {
     const RowMeta* meta;   // [nRowsTotal]
     const float* rowX;
     float2* hits;          // sorted (y,z) pairs
-    uint32_t* orig;        // sorted position -> load index
+    uint32_t* orig;        // sorted position -> event-global cluster id (gidBase of the row + load index)
     uint32_t* binStart;
     Bucket* buckets;       // [binCap], same indexing as binStart (row.binOff + bin)
     int32_t* linkUp;       // raw links, index = sorted position in the adjacent row
@@ -79,7 +79,8 @@ struct DevPtrs {
     uint32_t* weight;      // ownership key per hit
     int4* starts;          // (rowId, sorted position, sorted position of the linked hit in the row above, global id)
     TrackletRec* recs;
-    int32_t* rowHit;       // [maxTracklets][rhStride], sorted position of the tracklet's hit in each row, -1 none
+    int32_t* rowHit;       // [maxTracklets][rhStride], GLOBAL sorted position (row hitOff + position) of the tracklet's hit
+                           // in each row, -1 none: indexes weight[] / orig[] directly
     tpc_track* tracks;
     uint32_t* clusterIds;
     uint32_t* counters;

@@ -17,7 +17,10 @@ __device__ __forceinline__ int bin_of(float v, float v0, float inv, int n) {
 // ------------------------------------------------------------------------------------------ K1
 // One block per (sector,row): bounding box -> grid -> histogram in shared memory -> scan -> scatter.
 // Input: SoA y[], z[] as loaded (coalesced reads).  Output: sorted float2 (y,z), orig[], binStart[], grid.
-constexpr int kK1Threads = 256;
+#ifndef TPC_K1T
+#define TPC_K1T 256
+#endif
+constexpr int kK1Threads = TPC_K1T;
 
 __global__ void __launch_bounds__(kK1Threads) k1_sort_grid(DevPtrs d) {
     const int rowId = blockIdx.x;
@@ -126,7 +129,7 @@ __global__ void __launch_bounds__(kK1Threads) k1_sort_grid(DevPtrs d) {
         const int b = bin_of(c, z0, invZ, nZ) * nY + bin_of(a, y0, invY, nY);
         const uint32_t pos = atomicAdd(&sh[b], 1u);
         hs[pos] = make_float2(a, c);
-        og[pos] = (uint32_t)i;
+        og[pos] = M.gidBase + (uint32_t)i;
         wt[i] = 0u;
     }
     __syncthreads();
@@ -165,7 +168,10 @@ __device__ __forceinline__ void for_window(const RowGrid& R, const float2* __res
 
 // ------------------------------------------------------------------------------------------ K2
 // Neighbours finder (S2): for each hit the best (up,down) pair in rows r+1/r-1 by 3-point collinearity.
-constexpr int kK2Threads = 128;
+#ifndef TPC_K2T
+#define TPC_K2T 128
+#endif
+constexpr int kK2Threads = TPC_K2T;
 constexpr int kK2Cap = 16;   // down-candidates cached per thread; beyond that a nested rescan (slow, exact)
 
 __global__ void __launch_bounds__(kK2Threads) k2_neighbours(DevPtrs d, DevParams dp) {
@@ -244,7 +250,10 @@ __global__ void __launch_bounds__(kK2Threads) k2_neighbours(DevPtrs d, DevParams
 // Cleaner (S3): keep reciprocal links only.  Start hits (S4): no down-link, chain of >= seed_min_chain hits.
 // The chain test re-derives the cleaned up-links of the next rows from the raw links (same predicate), so one
 // kernel does both; the start list is appended with one atomic per warp (ballot + prefix).
-constexpr int kK3Threads = 128;
+#ifndef TPC_K3T
+#define TPC_K3T 64
+#endif
+constexpr int kK3Threads = TPC_K3T;
 
 __device__ __forceinline__ int clean_up_link(const DevPtrs& d, int hitOff, int hitOffUp, int i) {
     const int u = d.linkUp[hitOff + i];
@@ -258,7 +267,6 @@ __global__ void __launch_bounds__(kK3Threads) k3_clean_start(DevPtrs d, DevParam
     if (n == 0) return;
     const bool hasUp = r + 1 < dp.nRows, hasDn = r >= 1;
     const int hitOff = d.grid[rowId].hitOff;
-    const uint32_t gidBase = d.meta[rowId].gidBase;
     const int hitOffU = hasUp ? d.grid[rowId + 1].hitOff : hitOff;
     const int hitOffD = hasDn ? d.grid[rowId - 1].hitOff : hitOff;
     const unsigned lane = threadIdx.x & 31u;
@@ -291,7 +299,7 @@ __global__ void __launch_bounds__(kK3Threads) k3_clean_start(DevPtrs d, DevParam
             if (lane == 0) pos = atomicAdd(&d.counters[kNStart], (unsigned)__popc(m));
             pos = __shfl_sync(0xffffffffu, pos, 0) + __popc(m & ((1u << lane) - 1u));
             if (isStart && pos < (unsigned)d.maxTracklets)   // (row, hit, linked hit, canonical id): all K5 needs to begin
-                d.starts[pos] = make_int4(rowId, i, upKeep, (int)(gidBase + d.orig[hitOff + i]));
+                d.starts[pos] = make_int4(rowId, i, upKeep, (int)d.orig[hitOff + i]);
         }
     }
 #pragma unroll

@@ -242,14 +242,17 @@ __global__ void dump_links_kernel(DevPtrs d, int nRows, int64_t N, int32_t* out)
     const RowGrid R = d.grid[rowId];
     const RowMeta M = d.meta[rowId];
     for (int k = threadIdx.x; k < M.n; k += blockDim.x) {
-        const int64_t g = (int64_t)M.gidBase + d.orig[R.hitOff + k];
+        const int64_t g = (int64_t)d.orig[R.hitOff + k];
         const int32_t* src[4] = {d.linkUp, d.linkDn, d.linkUpC, d.linkDnC};
         for (int w = 0; w < 4; w++) {
             const int l = src[w][R.hitOff + k];
             int v = -1;
             if (l >= 0) {
                 const bool upw = (w % 2) == 0;
-                if ((upw && r + 1 < nRows) || (!upw && r >= 1)) v = (int)d.orig[d.grid[rowId + (upw ? 1 : -1)].hitOff + l];
+                if ((upw && r + 1 < nRows) || (!upw && r >= 1)) {
+                    const int nb = rowId + (upw ? 1 : -1);
+                    v = (int)(d.orig[d.grid[nb].hitOff + l] - d.meta[nb].gidBase);
+                }
             }
             out[(int64_t)w * N + g] = v;
         }
@@ -259,7 +262,7 @@ __global__ void dump_starts_kernel(DevPtrs d, unsigned n, uint32_t* out) {
     const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const int4 s = d.starts[i];
-    out[i] = d.meta[s.x].gidBase + d.orig[d.grid[s.x].hitOff + s.y];
+    out[i] = d.orig[d.grid[s.x].hitOff + s.y];
 }
 __global__ void dump_rowhit_kernel(DevPtrs d, int nRows, unsigned n, int32_t* out) {
     const unsigned slot = blockIdx.x;
@@ -269,7 +272,7 @@ __global__ void dump_rowhit_kernel(DevPtrs d, int nRows, unsigned n, int32_t* ou
         int v = -1;
         if (r >= t.firstRow && r <= t.lastRow) {
             const int h = d.rowHit[(size_t)slot * d.rhStride + r];
-            if (h >= 0) v = (int)d.orig[d.grid[t.sector * nRows + r].hitOff + h];
+            if (h >= 0) v = (int)(d.orig[h] - d.meta[t.sector * nRows + r].gidBase);
         }
         out[(size_t)slot * nRows + r] = v;
     }
@@ -281,7 +284,7 @@ __global__ void dump_owner_kernel(DevPtrs d, int nRows, uint32_t* out) {
     const uint32_t sb = d.sectorGidBase[rowId / nRows];
     for (int k = threadIdx.x; k < M.n; k += blockDim.x) {
         const uint32_t w = d.weight[R.hitOff + k];
-        out[M.gidBase + d.orig[R.hitOff + k]] = w ? sb + (0x00FFFFFFu - (w & 0x00FFFFFFu)) : 0xFFFFFFFFu;
+        out[d.orig[R.hitOff + k]] = w ? sb + (0x00FFFFFFu - (w & 0x00FFFFFFu)) : 0xFFFFFFFFu;
     }
 }
 
