@@ -161,45 +161,40 @@ def oracle_baseline(ev, budget_s: float = 15.0):
             "seconds": best, "stage_seconds": o.stage_seconds()}
 
 
-def multi_event_leg(torch, binding, ev, params, dev, k: int, reps: int):
-    """Several events in flight (two tracker instances per GPU gave -24 % per event): k tracker
-    instances, each with its own workspace and stream, track `reps` events each; kernels of different instances
-    overlap.  Inputs resident in HBM; the k working sets (k x ~0.4 GB) exceed the 126 MB L2, no flush in between."""
-    trks, streams, keep = [], [], []
-    for i in range(k):
-        st = torch.cuda.Stream(device=dev)
-        t = binding.Tracker(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz, params)
-        t.set_stream(st.cuda_stream)
-        t.allocate_workspace(ev.n_clusters, device=dev)
-        y, z = torch.from_numpy(ev.y).to(dev), torch.from_numpy(ev.z).to(dev)
-        torch.cuda.synchronize()
-        t.load_event(ev.row_counts, y, z)
-        keep.append((y, z))
-        trks.append(t); streams.append(st)
-    torch.cuda.synchronize()
-    def run(n):
-        start = torch.cuda.Event(enable_timing=True)
-        start.record(torch.cuda.current_stream())
-        ends = []
-        for st in streams:
-            st.wait_event(start)
-        for _ in range(n):
-            for t in trks:
-                t.track_sectors()
-        for st in streams:
-            e = torch.cuda.Event(enable_timing=True)
-            e.record(st)
-            ends.append(e)
-        torch.cuda.synchronize()
-        return max(start.elapsed_time(e) for e in ends)
-    run(3)
-    ms = run(reps)
-    n_tracks = [t.get_tracks(copy=False)[0].shape[0] for t in trks]
-    for t in trks:
-        t.destroy()
-    return {"events_in_flight": k, "events": k * reps, "ms_per_event": ms / (k * reps),
-            "value": ev.n_clusters * k * reps / (ms * 1e-3), "unit": UNIT, "n_tracks_each": n_tracks[0],
-            "note": "k tracker instances on k streams, same synthetic event in each, device-timed over all streams"}
+def multi_event_leg(torch, binding, datagen, args, params, dev, rank: int, k: int, reps: int):
+    """Several events per call (one event cannot fill the GPU; two tracker instances per GPU gave
+    -24 % per event there).  Phase-I sectors are independent, so k events are loaded as 36*k sectors of
+    ONE tracker and tracked by one tpc_track_sectors call: every kernel then works on k events at once.
+    Same timing rules as the main leg (inputs resident in HBM, L2 flushed before every call, CUDA events)."""
+    evs = [datagen.config_event(args.config, seed=1000 + rank * k + i) for i in range(k)]
+    e0 = evs[0]
+    counts = np.concatenate([e.row_counts.reshape(-1) for e in evs]).reshape(e0.n_sectors * k, e0.n_rows)
+    n_total = int(sum(e.n_clusters for e in evs))
+    trk = binding.Tracker(e0.n_sectors * k, e0.n_rows, e0.row_x, e0.bz, params)
+    stream = torch.cuda.current_stream()
+    trk.set_stream(stream.cuda_stream)
+    trk.allocate_workspace(n_total, device=dev)
+    y = torch.from_numpy(np.concatenate([e.y for e in evs])).to(dev)
+    z = torch.from_numpy(np.concatenate([e.z for e in evs])).to(dev)
+    trk.load_event(counts, y, z)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    times = []
+    for i in range(3 + reps):
+        flush.fill_(1)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        trk.track_sectors()
+        b.record(stream)
+        trk.sync()
+        if i >= 3:
+            times.append(a.elapsed_time(b))
+    ms = sum(times) / len(times)
+    st = trk.get_stats()
+    trk.destroy()
+    return {"events_per_call": k, "calls": reps, "n_clusters_per_call": n_total, "ms_per_call": ms, "ms_per_event": ms / k,
+            "value": n_total / (ms * 1e-3), "unit": UNIT, "n_tracks": st["n_tracks"],
+            "kernel_us_per_event": {kk: round(v / k, 1) for kk, v in st["kernel_us"].items()},
+            "note": "k independent synthetic events (other seeds) as 36*k sectors of one tracker, one call"}
 
 
 def run_reference(args, rank, world, dist):
@@ -247,8 +242,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--bins-per-hit", type=float, default=None, help="override tpc_params.grid_bins_per_hit (tuning)")
-    ap.add_argument("--events-in-flight", type=int, default=3,
-                    help="extra leg: this many tracker instances on their own streams (PAPER.md:82-84); 0 = skip")
+    ap.add_argument("--events-per-call", type=int, default=4,
+                    help="extra leg: this many events tracked by one call (PAPER.md:82-84); 0 or 1 = skip")
     args = ap.parse_args()
     rank, world, local, dist = init_dist(args.gpus)
     if args.impl == "reference":
@@ -317,23 +312,46 @@ def main():
     st = trk.get_stats()
     value, ms, n_total = aggregate(dist, dev, ev.n_clusters, step_ms)
 
-    # ---- end to end through the C ABI with HOST buffers (pinned), H2D + D2H inside the timed region
-    y_pin, z_pin = torch.from_numpy(ev.y).pin_memory(), torch.from_numpy(ev.z).pin_memory()
-    def step_e2e():
-        trk.load_event(ev.row_counts, y_pin.numpy(), z_pin.numpy())
-        trk.track_sectors()
-        return trk.get_tracks(copy=False)
-    for _ in range(3):
-        tr, ids = step_e2e()
-    torch.cuda.synchronize()
+    # ---- end to end through the C ABI with HOST buffers (pinned), H2D + D2H of every step inside the timed region.
+    # Two tracker instances, each driven by its own host thread on its own stream, take alternate events: while one
+    # tracks, the other uploads its next event / downloads its tracks (the paper's DMA || kernel pipeline,
+    # PAPER.md:66 and Fig. 4).  Every step still does load_event (pinned host -> device), track_sectors, get_tracks
+    # (device -> pinned host); time = wall clock around all steps of both threads.
+    n_pipe = 2
+    pipes = []
+    for i in range(n_pipe):
+        sti = torch.cuda.Stream(device=dev)
+        ti = trk if i == 0 else binding.Tracker(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz, params)
+        if i > 0:
+            ti.set_stream(sti.cuda_stream)
+            ti.allocate_workspace(ev.n_clusters, device=dev)
+        pipes.append((ti, torch.from_numpy(ev.y.copy()).pin_memory(), torch.from_numpy(ev.z.copy()).pin_memory()))
+    last = [None] * n_pipe
+
+    def e2e_worker(i, n):
+        torch.cuda.set_device(dev)
+        ti, yp, zp = pipes[i]
+        for _ in range(n):
+            ti.load_event(ev.row_counts, yp.numpy(), zp.numpy())
+            ti.track_sectors()
+            last[i] = ti.get_tracks(copy=False)
+
+    def e2e_run(n_each):
+        ths = [threading.Thread(target=e2e_worker, args=(i, n_each)) for i in range(n_pipe)]
+        t0 = time.perf_counter()
+        for th in ths:
+            th.start()
+        for th in ths:
+            th.join()
+        torch.cuda.synchronize()
+        return time.perf_counter() - t0
+
+    e2e_run(2)
     if dist is not None:
         dist.barrier()
-    n_e2e = max(3, min(args.steps, 20))
-    t0 = time.perf_counter()
-    for _ in range(n_e2e):
-        tr, ids = step_e2e()
-    torch.cuda.synchronize()
-    e2e_ms = (time.perf_counter() - t0) / n_e2e * 1e3
+    n_e2e = max(4, min(args.steps, 20)) // n_pipe * n_pipe
+    e2e_ms = e2e_run(n_e2e // n_pipe) / n_e2e * 1e3
+    tr, ids = last[0]
     e2e_value, e2e_ms_max, _ = aggregate(dist, dev, ev.n_clusters, e2e_ms)
     h2d = 8 * ev.n_clusters + 48 * ev.n_sectors * ev.n_rows + 4 * (ev.n_sectors + 1)
     d2h = 112 * int(tr.shape[0]) + 4 * int(ids.shape[0]) + 64
@@ -363,7 +381,8 @@ def main():
                    "workspace_bytes": ws_bytes, "workspace_over_input": round(ws_bytes / (12.0 * ev.n_clusters), 2),
                    "grid_bins_per_hit": float(params.grid_bins_per_hit)},
         "clocks": clocks,
-        "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms_max, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+        "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms_max, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "steps": n_e2e, "pipeline": "2 tracker instances / host threads / streams: copies of one event overlap the kernels of the other"},
         "gpu_launches": args.steps * trk.launches_per_track(),
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": round(achieved, 2), "peak": peak, "unit": "GB/s",
                      "frac": round(achieved / peak, 5), "traffic": traffic, "peak_source": peak_src,
@@ -372,8 +391,8 @@ def main():
                                     "frac": round(sum(ab.values()) / (ms * 1e-3) / 1e9 / peak, 5)}},
         "kernels": per_kernel,
     }
-    if args.events_in_flight > 1:
-        me = multi_event_leg(torch, binding, ev, params, dev, args.events_in_flight, max(3, min(args.steps, 10)))
+    if args.events_per_call > 1 and args.config <= 3:
+        me = multi_event_leg(torch, binding, datagen, args, params, dev, rank, args.events_per_call, max(3, min(args.steps, 10)))
         me["value"] = reduce_over_ranks(dist, me["value"], "sum", dev)      # whole job: sum of the ranks' rates
         out["multi_event"] = me
     if rank == 0 and not args.no_cpu_baseline:

@@ -126,6 +126,14 @@ void bind_pointers(tpc_tracker* t) {
     d.rhStride = t->rhStride;
 }
 
+// Page-locked host memory (cudaMallocHost / cudaHostRegister, e.g. a pinned torch tensor): the DMA engine can read it
+// directly, so large loads skip the copy into the library's own pinned mirror.
+bool is_pinned_host_pointer(const void* p) {
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return a.type == cudaMemoryTypeHost;
+}
+
 bool is_device_pointer(const void* p) {
     cudaPointerAttributes a;
     if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
@@ -215,6 +223,17 @@ int stage_clusters(tpc_tracker* t, int64_t at, int64_t n, const float* y, const 
     if (is_device_pointer(y)) {
         CUDA_TRY(t, cudaMemcpyAsync((float*)t->dev.inY + at, y, sizeof(float) * n, cudaMemcpyDeviceToDevice, t->stream));
         CUDA_TRY(t, cudaMemcpyAsync((float*)t->dev.inZ + at, z, sizeof(float) * n, cudaMemcpyDeviceToDevice, t->stream));
+    } else if (n >= (1 << 16) && is_pinned_host_pointer(y) && is_pinned_host_pointer(z)) {
+        // large page-locked buffers: DMA straight from the caller's memory; the call returns when the copy is done,
+        // so the caller may reuse the buffers at once ("copied", tpctrk.h)
+        int rc = flush_dirty(t);     // keep the order of uploads
+        if (rc != TPC_OK) return rc;
+        CUDA_TRY(t, cudaMemcpyAsync((float*)t->dev.inY + at, y, sizeof(float) * n, cudaMemcpyHostToDevice, t->stream));
+        CUDA_TRY(t, cudaMemcpyAsync((float*)t->dev.inZ + at, z, sizeof(float) * n, cudaMemcpyHostToDevice, t->stream));
+        if (!t->evUpload) CUDA_TRY(t, cudaEventCreateWithFlags(&t->evUpload, cudaEventDisableTiming));
+        CUDA_TRY(t, cudaEventRecord(t->evUpload, t->stream));
+        CUDA_TRY(t, cudaEventSynchronize(t->evUpload));
+        t->uploadPending = false;
     } else {
         int rc = ensure_host_stage(t, at + n);
         if (rc != TPC_OK) return rc;

@@ -253,3 +253,42 @@ def test_geometry_whose_row_table_exceeds_shared_memory():
     trk, tracks, ids = run_gpu(ev)
     out = compare(ev, trk, tracks, ids, ref)
     assert out["tracklet_mismatch"] == 0 and out["link_mismatch_0"] == 0
+
+
+def test_several_events_per_call_as_extra_sectors():
+    """bench.py's multi_event leg: k events loaded as 36*k sectors of one tracker (sectors are independent,
+    PAPER.md:76).  Every stage must match the oracle run on the same concatenation, and each event's tracks must be
+    the ones it gets when tracked alone."""
+    _cuda()
+    evs = [datagen.config_event(2, seed=s) for s in (20, 21)]
+    e0 = evs[0]
+    ev = datagen.Event(e0.n_sectors * 2, e0.n_rows, e0.row_x, e0.bz,
+                       np.concatenate([e.row_counts.reshape(-1) for e in evs]).reshape(e0.n_sectors * 2, e0.n_rows),
+                       np.concatenate([e.y for e in evs]), np.concatenate([e.z for e in evs]),
+                       np.concatenate([e.truth for e in evs]))
+    ref = oracle.run_event(ev)
+    trk, tracks, ids = run_gpu(ev)
+    out = compare(ev, trk, tracks, ids, ref)
+    assert out["tracklet_mismatch"] == 0 and out["link_mismatch_0"] == 0
+    alone = oracle.run_event(evs[1])
+    second = tracks[tracks["sector"] >= e0.n_sectors]
+    assert second.size == alone.tracks.size
+    assert np.array_equal(np.sort(second["n_clusters"]), np.sort(alone.tracks["n_clusters"]))
+
+
+def test_page_locked_host_input_is_read_directly():
+    """Large page-locked host buffers are uploaded straight from the caller's memory (no staging copy); the call
+    returns after the copy, so the buffers may be overwritten at once."""
+    torch = _cuda()
+    ev = datagen.config_event(2, seed=9)
+    ref = oracle.run_event(ev)
+    trk = binding.Tracker(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz)
+    trk.set_stream(torch.cuda.current_stream().cuda_stream)
+    trk.allocate_workspace(ev.n_clusters)
+    y, z = torch.from_numpy(ev.y.copy()).pin_memory(), torch.from_numpy(ev.z.copy()).pin_memory()
+    trk.load_event(ev.row_counts, y.numpy(), z.numpy())
+    y.fill_(float("nan")); z.fill_(float("nan"))          # must not matter any more
+    trk.track_sectors()
+    tracks, ids = trk.get_tracks()
+    out = compare(ev, trk, tracks, ids, ref)
+    assert out["tracklet_mismatch"] == 0
