@@ -172,9 +172,15 @@ __device__ __forceinline__ void for_window(const RowGrid& R, const float2* __res
 #define TPC_K2T 128
 #endif
 constexpr int kK2Threads = TPC_K2T;
-constexpr int kK2Cap = 16;   // down-candidates cached per thread; beyond that a nested rescan (slow, exact)
+#ifndef TPC_K2CAP
+#define TPC_K2CAP 8
+#endif
+constexpr int kK2Cap = TPC_K2CAP;   // down-candidates cached per thread; beyond that a nested rescan (slow, exact)
 
-__global__ void __launch_bounds__(kK2Threads) k2_neighbours(DevPtrs d, DevParams dp) {
+#ifndef TPC_K2B
+#define TPC_K2B 8
+#endif
+__global__ void __launch_bounds__(kK2Threads, TPC_K2B) k2_neighbours(DevPtrs d, DevParams dp) {
     const int rowId = blockIdx.x;
     const int r = rowId % dp.nRows;
     const int n = d.meta[rowId].n;
