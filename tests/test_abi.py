@@ -27,12 +27,13 @@ def test_library_exports_every_declared_symbol():
 
 
 def test_struct_layouts_match_header():
-    assert ctypes.sizeof(binding.tpc_params) == 16 * 4
+    assert ctypes.sizeof(binding.tpc_params) == 17 * 4
     assert ctypes.sizeof(binding.tpc_stats) == 10 * 8 + 8 * 4
     assert binding.TRACK_DTYPE.itemsize == 112
     p = binding.default_params()
     assert abs(p.err2_y - 0.01) < 1e-9 and p.min_hits == 10 and p.max_gap == 4 and p.seed_min_chain == 3
     assert abs(p.nf_tz - 1.5) < 1e-9 and abs(p.kf_ckk0 - 100.0) < 1e-9 and abs(p.road_max - 2.0) < 1e-9
+    assert abs(p.max_tracklets_per_cluster - 0.125) < 1e-9 and abs(p.grid_bins_per_hit - 4.0) < 1e-9
 
 
 def test_create_validates_geometry():
