@@ -267,8 +267,12 @@ __device__ __forceinline__ int clean_up_link(const DevPtrs& d, int hitOff, int h
 }
 
 __global__ void __launch_bounds__(kK3Threads) k3_clean_start(DevPtrs d, DevParams dp) {
-    const int rowId = blockIdx.x;
-    const int r = rowId % dp.nRows;
+    // Blocks run pad row by pad row (all sectors of row 0, then row 1, ...): blocks are dispatched in index order, so
+    // the start list comes out roughly ordered by pad row.  K5 gives 32 consecutive start hits to a warp; tracklets
+    // that start in the same row are in the same leg at the same time far more often than random ones, so the lanes
+    // of a warp finish together (fewer half-empty warp steps).  Nothing depends on the order.
+    const int r = blockIdx.x / dp.nSec;
+    const int rowId = (blockIdx.x - r * dp.nSec) * dp.nRows + r;
     const int n = d.meta[rowId].n;
     if (n == 0) return;
     const bool hasUp = r + 1 < dp.nRows, hasDn = r >= 1;
