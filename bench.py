@@ -313,11 +313,11 @@ def main():
     value, ms, n_total = aggregate(dist, dev, ev.n_clusters, step_ms)
 
     # ---- end to end through the C ABI with HOST buffers (pinned), H2D + D2H of every step inside the timed region.
-    # Two tracker instances, each driven by its own host thread on its own stream, take alternate events: while one
-    # tracks, the other uploads its next event / downloads its tracks (the paper's DMA || kernel pipeline,
+    # Three tracker instances, each driven by its own host thread on its own stream, take events in turn: while one
+    # tracks, the others upload their next event / download their tracks (the paper's DMA || kernel pipeline,
     # PAPER.md:66 and Fig. 4).  Every step still does load_event (pinned host -> device), track_sectors, get_tracks
     # (device -> pinned host); time = wall clock around all steps of both threads.
-    n_pipe = 2
+    n_pipe = 3      # measured on config 3: 2 / 3 / 4 instances -> 0.99 / 0.76 / 0.84 ms per event
     pipes = []
     for i in range(n_pipe):
         sti = torch.cuda.Stream(device=dev)
@@ -382,7 +382,7 @@ def main():
                    "grid_bins_per_hit": float(params.grid_bins_per_hit)},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms_max, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "steps": n_e2e, "pipeline": "2 tracker instances / host threads / streams: copies of one event overlap the kernels of the other"},
+                "steps": n_e2e, "pipeline": "3 tracker instances / host threads / streams: copies of one event overlap the kernels of the others"},
         "gpu_launches": args.steps * trk.launches_per_track(),
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": round(achieved, 2), "peak": peak, "unit": "GB/s",
                      "frac": round(achieved / peak, 5), "traffic": traffic, "peak_source": peak_src,
