@@ -41,6 +41,7 @@ __global__ void __launch_bounds__(kK1Threads) k1_sort_grid(DevPtrs d) {
     }
     extern __shared__ uint32_t sh[];            // [maxBins + 1] histogram / cursors
     __shared__ float redA[4][kK1Threads / 32];
+    __shared__ float redZ[kK1Threads / 32];
     __shared__ uint32_t warpSum[kK1Threads / 32];
     __shared__ int sNY, sNZ;
     __shared__ float sY0, sZ0, sInvY, sInvZ;
@@ -49,28 +50,42 @@ __global__ void __launch_bounds__(kK1Threads) k1_sort_grid(DevPtrs d) {
 
     // 1. bounding box
     float ymin = 3.0e38f, ymax = -3.0e38f, zmin = 3.0e38f, zmax = -3.0e38f;
+    float zsum = 0.0f;
     for (int i = tid; i < n; i += kK1Threads) {
         const float a = y[i], b = z[i];
         ymin = fminf(ymin, a); ymax = fmaxf(ymax, a);
         zmin = fminf(zmin, b); zmax = fmaxf(zmax, b);
+        zsum += b;
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
+        zsum += __shfl_xor_sync(0xffffffffu, zsum, o);
         ymin = fminf(ymin, __shfl_xor_sync(0xffffffffu, ymin, o));
         ymax = fmaxf(ymax, __shfl_xor_sync(0xffffffffu, ymax, o));
         zmin = fminf(zmin, __shfl_xor_sync(0xffffffffu, zmin, o));
         zmax = fmaxf(zmax, __shfl_xor_sync(0xffffffffu, zmax, o));
     }
-    if ((tid & 31) == 0) { redA[0][tid >> 5] = ymin; redA[1][tid >> 5] = ymax; redA[2][tid >> 5] = zmin; redA[3][tid >> 5] = zmax; }
+    if ((tid & 31) == 0) { redA[0][tid >> 5] = ymin; redA[1][tid >> 5] = ymax; redA[2][tid >> 5] = zmin; redA[3][tid >> 5] = zmax; redZ[tid >> 5] = zsum; }
     __syncthreads();
     if (tid == 0) {
         for (int w = 1; w < kK1Threads / 32; w++) {
             ymin = fminf(ymin, redA[0][w]); ymax = fmaxf(ymax, redA[1][w]);
             zmin = fminf(zmin, redA[2][w]); zmax = fmaxf(zmax, redA[3][w]);
+            zsum += redZ[w];
         }
         // non-finite input must not blow the grid up
         ymin = fminf(fmaxf(ymin, -1.0e4f), 1.0e4f); ymax = fminf(fmaxf(ymax, -1.0e4f), 1.0e4f);
         zmin = fminf(fmaxf(zmin, -1.0e4f), 1.0e4f); zmax = fminf(fmaxf(zmax, -1.0e4f), 1.0e4f);
+        // The grid need not cover every hit: bin_of clamps, so hits (and queries) beyond the grid's range fall into
+        // its edge bins.  In z the occupancy is lopsided - tracks fill |z| < ~x, noise the whole drift length - so
+        // the z-range is cut to 2.2 x the distance from the denser end to the mean: the bins get finer where the
+        // tracks are, for the same number of bins (a uniform or symmetric distribution keeps its full range).
+        const float zmean = zsum / (float)n;
+        if (zmean > zmin && zmean < zmax) {
+            const float a = zmean - zmin, b = zmax - zmean;
+            if (a < b) zmax = fminf(zmax, zmin + 2.2f * a);
+            else zmin = fmaxf(zmin, zmax - 2.2f * b);
+        }
         const float spanY = fmaxf(ymax - ymin, 1.0e-2f), spanZ = fmaxf(zmax - zmin, 1.0e-2f);
         // kBinsPerHit bins per hit, bins twice as long in z as in y (a query costs per z-bin-row), >= 0.5 cm
         const int target = max(1, M.maxBins);
