@@ -17,6 +17,9 @@ __device__ __forceinline__ int bin_of(float v, float v0, float inv, int n) {
 // ------------------------------------------------------------------------------------------ K1
 // One block per (sector,row): bounding box -> grid -> histogram in shared memory -> scan -> scatter.
 // Input: SoA y[], z[] as loaded (coalesced reads).  Output: sorted float2 (y,z), orig[], binStart[], grid.
+#ifndef TPC_ZF
+#define TPC_ZF 2.4f   /* measured on config 3 (K5 us): 1.5 -> 847, 1.8 -> 590, 2.2 -> 497, 2.6 -> 509; the steep side is the low one */
+#endif
 #ifndef TPC_K1T
 #define TPC_K1T 256
 #endif
@@ -78,13 +81,13 @@ __global__ void __launch_bounds__(kK1Threads) k1_sort_grid(DevPtrs d) {
         zmin = fminf(fmaxf(zmin, -1.0e4f), 1.0e4f); zmax = fminf(fmaxf(zmax, -1.0e4f), 1.0e4f);
         // The grid need not cover every hit: bin_of clamps, so hits (and queries) beyond the grid's range fall into
         // its edge bins.  In z the occupancy is lopsided - tracks fill |z| < ~x, noise the whole drift length - so
-        // the z-range is cut to 2.2 x the distance from the denser end to the mean: the bins get finer where the
+        // the z-range is cut to TPC_ZF x the distance from the denser end to the mean: the bins get finer where the
         // tracks are, for the same number of bins (a uniform or symmetric distribution keeps its full range).
         const float zmean = zsum / (float)n;
         if (zmean > zmin && zmean < zmax) {
             const float a = zmean - zmin, b = zmax - zmean;
-            if (a < b) zmax = fminf(zmax, zmin + 2.2f * a);
-            else zmin = fmaxf(zmin, zmax - 2.2f * b);
+            if (a < b) zmax = fminf(zmax, zmin + TPC_ZF * a);
+            else zmin = fmaxf(zmin, zmax - TPC_ZF * b);
         }
         const float spanY = fmaxf(ymax - ymin, 1.0e-2f), spanZ = fmaxf(zmax - zmin, 1.0e-2f);
         // kBinsPerHit bins per hit, bins twice as long in z as in y (a query costs per z-bin-row), >= 0.5 cm
