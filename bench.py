@@ -157,8 +157,26 @@ def oracle_baseline(ev, budget_s: float = 15.0):
         t0 = time.perf_counter()
         o.run(sample.row_counts, sample.y, sample.z, fetch=False)
         best = min(best, time.perf_counter() - t0)
-    return {"value": sample.n_clusters / best, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc,
-            "seconds": best, "stage_seconds": o.stage_seconds()}
+    out = {"value": sample.n_clusters / best, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc,
+           "seconds": best, "stage_seconds": o.stage_seconds()}
+    # the SAME single-threaded oracle, one instance per sector, on a pool of P host
+    # threads (sectors are independent; ctypes releases the GIL).  Context next to the 1-core number.
+    try:
+        from concurrent.futures import ThreadPoolExecutor
+        p = len(os.sched_getaffinity(0))
+        subs = [sample.sector_slice(s) for s in range(sample.n_sectors)]
+        if p > 1 and len(subs) > 1:
+            def one(sub):
+                oracle.Oracle(1, sub.n_rows, sub.row_x, sub.bz).run(sub.row_counts, sub.y, sub.z, fetch=False)
+            with ThreadPoolExecutor(max_workers=p) as ex:
+                t0 = time.perf_counter()
+                list(ex.map(one, subs))
+                dt = time.perf_counter() - t0
+            out["all_cores"] = {"value": sample.n_clusters / dt, "unit": UNIT, "cores": min(p, len(subs)),
+                                "seconds": dt, "how": "one oracle instance per sector on a thread pool"}
+    except Exception as e:      # the 1-core number is the contract; this one is context
+        out["all_cores"] = {"error": str(e)}
+    return out
 
 
 def multi_event_leg(torch, binding, datagen, args, params, dev, rank: int, k: int, reps: int):
