@@ -184,6 +184,48 @@ __device__ __forceinline__ void for_window(const RowGrid& R, const float2* __res
     }
 }
 
+// The same enumeration in two steps, for K2: win_ranges() requests the bin-table entries of up to three z-rows of
+// bins at once (six independent loads; both adjacent rows' windows are requested before either is scanned), scan_ranges()
+// then walks the hit ranges.  Windows taller than three bin rows take the generic loop.
+struct WinRanges {
+    int k0[3], k1[3];
+    int by0, by1, bz0, bz1;
+};
+__device__ __forceinline__ WinRanges win_ranges(const RowGrid& R, const uint32_t* __restrict__ binStart, float yc,
+                                                float zc, float wy, float wz) {
+    WinRanges w;
+    w.by0 = bin_of(yc - wy - kGridMargin, R.y0, R.invY, R.nY);
+    w.by1 = bin_of(yc + wy + kGridMargin, R.y0, R.invY, R.nY);
+    w.bz0 = bin_of(zc - wz - kGridMargin, R.z0, R.invZ, R.nZ);
+    w.bz1 = bin_of(zc + wz + kGridMargin, R.z0, R.invZ, R.nZ);
+    const uint32_t* __restrict__ bs = binStart + R.binOff;
+#pragma unroll
+    for (int j = 0; j < 3; j++) {
+        const int bz = min(w.bz0 + j, w.bz1);           // rows beyond the window repeat the last one (valid address)
+        const bool in = w.bz0 + j <= w.bz1;
+        const int a = (int)bs[bz * R.nY + w.by0], b = (int)bs[bz * R.nY + w.by1 + 1];
+        w.k0[j] = in ? a : 0;
+        w.k1[j] = in ? b : 0;
+    }
+    return w;
+}
+template <class F>
+__device__ __forceinline__ void scan_ranges(const WinRanges& w, const RowGrid& R, const float2* __restrict__ hits,
+                                            const uint32_t* __restrict__ binStart, F&& f) {
+    const float2* __restrict__ hs = hits + R.hitOff;
+    if (w.bz1 - w.bz0 <= 2) {
+#pragma unroll
+        for (int j = 0; j < 3; j++)
+            for (int k = w.k0[j]; k < w.k1[j]; k++) f(k, hs[k]);
+    } else {
+        const uint32_t* __restrict__ bs = binStart + R.binOff;
+        for (int bz = w.bz0; bz <= w.bz1; bz++) {
+            const int k0 = (int)bs[bz * R.nY + w.by0], k1 = (int)bs[bz * R.nY + w.by1 + 1];
+            for (int k = k0; k < k1; k++) f(k, hs[k]);
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------ K2
 // Neighbours finder (S2): for each hit the best (up,down) pair in rows r+1/r-1 by 3-point collinearity.
 #ifndef TPC_K2T
@@ -230,7 +272,9 @@ __global__ void __launch_bounds__(kK2Threads, TPC_K2B) k2_neighbours(DevPtrs d, 
         float cy[kK2Cap], cz[kK2Cap];
         int ck[kK2Cap];
         int nd = 0;
-        for_window(Rd, d.hits, d.binStart, h.x, h.y, wyD, wzD, [&](int k, float2 c) {
+        const WinRanges rD = win_ranges(Rd, d.binStart, h.x, h.y, wyD, wzD);
+        const WinRanges rU = win_ranges(Ru, d.binStart, h.x, h.y, wyU, wzU);
+        scan_ranges(rD, Rd, d.hits, d.binStart, [&](int k, float2 c) {
             if (fabsf(c.x - h.x) <= wyD && fabsf(c.y - h.y) <= wzD) {
                 if (nd < kK2Cap) { cy[nd] = wd * c.x; cz[nd] = wd * c.y; ck[nd] = k; }
                 nd++;
@@ -247,7 +291,7 @@ __global__ void __launch_bounds__(kK2Threads, TPC_K2B) k2_neighbours(DevPtrs d, 
             if (better) { best = d2; bestU = ku; bestD = kd; }
         };
         if (nd > 0) {
-            for_window(Ru, d.hits, d.binStart, h.x, h.y, wyU, wzU, [&](int ku, float2 c) {
+            scan_ranges(rU, Ru, d.hits, d.binStart, [&](int ku, float2 c) {
                 if (!(fabsf(c.x - h.x) <= wyU && fabsf(c.y - h.y) <= wzU)) return;
                 const float py = wu * c.x, pz = wu * c.y;
                 if (nd <= kK2Cap) {
