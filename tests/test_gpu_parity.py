@@ -292,3 +292,33 @@ def test_page_locked_host_input_is_read_directly():
     tracks, ids = trk.get_tracks()
     out = compare(ev, trk, tracks, ids, ref)
     assert out["tracklet_mismatch"] == 0
+
+
+def test_four_central_events_per_call_sampled_sectors():
+    """bench.py's multi_event leg at its full size and launch configuration: four config-3 events (seeds as in
+    bench.py) as 144 sectors of one tracker.  The oracle recomputes three sampled sectors (sectors are independent)."""
+    _cuda()
+    k = 4
+    evs = [datagen.config_event(3, seed=1000 + i) for i in range(k)]
+    e0 = evs[0]
+    ev = datagen.Event(e0.n_sectors * k, e0.n_rows, e0.row_x, e0.bz,
+                       np.concatenate([e.row_counts.reshape(-1) for e in evs]).reshape(e0.n_sectors * k, e0.n_rows),
+                       np.concatenate([e.y for e in evs]), np.concatenate([e.z for e in evs]),
+                       np.concatenate([e.truth for e in evs]))
+    trk, tracks, ids = run_gpu(ev)
+    assert np.unique(ids).size == ids.size and tracks["n_clusters"].min() >= 10
+    base = ev.row_base
+    for s in (5, 36 + 20, 3 * 36 + 35):
+        ref = oracle.run_event(ev.sector_slice(s))
+        g0 = int(base[s * ev.n_rows])
+        tg = tracks[tracks["sector"] == s]
+        assert tg.size == ref.tracks.size
+        key_g = ids[tg["cluster_offset"]].astype(np.int64) - g0
+        key_o = ref.cluster_ids[ref.tracks["cluster_offset"]].astype(np.int64)
+        tg, to = tg[np.argsort(key_g)], ref.tracks[np.argsort(key_o)]
+        assert np.array_equal(np.sort(key_g), np.sort(key_o))
+        for f in ("n_clusters", "first_row", "last_row", "n_fit"):
+            assert np.array_equal(tg[f], to[f]), f
+        for f in ("x", "p", "c", "chi2"):
+            a, b = tg[f].astype(np.float64), to[f]
+            assert np.all(np.abs(a - b) <= 1e-5 + 1e-4 * np.abs(b)), f
