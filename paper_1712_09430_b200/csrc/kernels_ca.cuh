@@ -24,6 +24,7 @@ __device__ __forceinline__ int bin_of(float v, float v0, float inv, int n) {
 #define TPC_K1T 256
 #endif
 constexpr int kK1Threads = TPC_K1T;
+constexpr int kK1Stage = 512;     // 8 KB of static shared memory beside the <= 32 KB dynamic histogram (48 KB limit)
 
 __global__ void __launch_bounds__(kK1Threads) k1_sort_grid(DevPtrs d) {
     const int rowId = blockIdx.x;
@@ -45,6 +46,12 @@ __global__ void __launch_bounds__(kK1Threads) k1_sort_grid(DevPtrs d) {
     extern __shared__ uint32_t sh[];            // [maxBins + 1] histogram / cursors
     __shared__ float redA[4][kK1Threads / 32];
     __shared__ float redZ[kK1Threads / 32];
+    // rows of up to kK1Stage hits keep their input and their sorted hits in shared memory, so that the three passes
+    // over the input and the bucket pass do not go back to global memory (each pass is one more dependent memory
+    // round trip in a block's life); larger rows re-read global memory
+    __shared__ float2 sIn[kK1Stage];
+    __shared__ float2 sSorted[kK1Stage];
+    const bool staged = n <= kK1Stage;
     __shared__ uint32_t warpSum[kK1Threads / 32];
     __shared__ int sNY, sNZ;
     __shared__ float sY0, sZ0, sInvY, sInvZ;
@@ -59,6 +66,7 @@ __global__ void __launch_bounds__(kK1Threads) k1_sort_grid(DevPtrs d) {
         ymin = fminf(ymin, a); ymax = fmaxf(ymax, a);
         zmin = fminf(zmin, b); zmax = fmaxf(zmax, b);
         zsum += b;
+        if (staged) sIn[i] = make_float2(a, b);
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
@@ -109,7 +117,8 @@ __global__ void __launch_bounds__(kK1Threads) k1_sort_grid(DevPtrs d) {
     for (int b = tid; b <= nBins; b += kK1Threads) sh[b] = 0u;
     __syncthreads();
     for (int i = tid; i < n; i += kK1Threads) {
-        const int b = bin_of(z[i], z0, invZ, nZ) * nY + bin_of(y[i], y0, invY, nY);
+        const float2 v = staged ? sIn[i] : make_float2(y[i], z[i]);
+        const int b = bin_of(v.y, z0, invZ, nZ) * nY + bin_of(v.x, y0, invY, nY);
         atomicAdd(&sh[b], 1u);
     }
     __syncthreads();
@@ -143,10 +152,12 @@ __global__ void __launch_bounds__(kK1Threads) k1_sort_grid(DevPtrs d) {
     uint32_t* __restrict__ og = d.orig + R.hitOff;
     uint32_t* __restrict__ wt = d.weight + R.hitOff;
     for (int i = tid; i < n; i += kK1Threads) {
-        const float a = y[i], c = z[i];
+        const float2 v = staged ? sIn[i] : make_float2(y[i], z[i]);
+        const float a = v.x, c = v.y;
         const int b = bin_of(c, z0, invZ, nZ) * nY + bin_of(a, y0, invY, nY);
         const uint32_t pos = atomicAdd(&sh[b], 1u);
         hs[pos] = make_float2(a, c);
+        if (staged) sSorted[pos] = make_float2(a, c);
         og[pos] = M.gidBase + (uint32_t)i;
         wt[i] = 0u;
     }
@@ -158,9 +169,9 @@ __global__ void __launch_bounds__(kK1Threads) k1_sort_grid(DevPtrs d) {
     for (int b = tid; b < nBins; b += kK1Threads) {
         const uint32_t s0 = b ? sh[b - 1] : 0u, cnt = sh[b] - s0;
         float2 h0 = make_float2(qnan, qnan), h1 = h0, h2 = h0;   // NaN never passes a window test
-        if (cnt > 0) h0 = hs[s0];
-        if (cnt > 1) h1 = hs[s0 + 1];
-        if (cnt > 2) h2 = hs[s0 + 2];
+        if (cnt > 0) h0 = staged ? sSorted[s0] : hs[s0];
+        if (cnt > 1) h1 = staged ? sSorted[s0 + 1] : hs[s0 + 1];
+        if (cnt > 2) h2 = staged ? sSorted[s0 + 2] : hs[s0 + 2];
         float4* q = reinterpret_cast<float4*>(bk + b);
         q[0] = make_float4(__uint_as_float(s0), __uint_as_float(cnt), h0.x, h0.y);
         q[1] = make_float4(h1.x, h1.y, h2.x, h2.y);
