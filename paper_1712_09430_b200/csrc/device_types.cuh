@@ -77,7 +77,10 @@ struct DevPtrs {
     int32_t* linkUpC;      // cleaned links
     int32_t* linkDnC;
     uint32_t* weight;      // ownership key per hit
-    int4* starts;          // (rowId, sorted position, sorted position of the linked hit in the row above, global id)
+    int4* startsRaw;       // K3/K4 output in append order: (rowId, sorted position, sorted position of the linked hit in the
+                           // row above, global id)
+    int4* starts;          // the same, ordered by pad row of the start hit (k4_sort_starts): K5's input
+    uint32_t* rowHist;     // [2][kMaxRows + 1]: start hits per pad row, scatter cursors
     TrackletRec* recs;
     int32_t* rowHit;       // [maxTracklets][rhStride], GLOBAL sorted position (row hitOff + position) of the tracklet's hit
                            // in each row, -1 none: indexes weight[] / orig[] directly

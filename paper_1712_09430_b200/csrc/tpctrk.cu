@@ -21,7 +21,7 @@ constexpr size_t kAlign = 256;
 inline size_t align_up(size_t v, size_t a = kAlign) { return (v + a - 1) / a * a; }
 
 struct Layout {   // byte offsets into the workspace
-    size_t inY, inZ, grid, meta, rowX, hits, orig, binStart, buckets, linkUp, linkDn, linkUpC, linkDnC, weight, starts, recs, rowHit,
+    size_t inY, inZ, grid, meta, rowX, hits, orig, binStart, buckets, linkUp, linkDn, linkUpC, linkDnC, weight, starts, startsRaw, rowHist, recs, rowHit,
         tracks, clusterIds, counters, sectorGidBase, total;
     int64_t hitCap, binCap, maxTracklets;
 };
@@ -64,7 +64,7 @@ struct tpc_tracker {
     cudaEvent_t ev[8] = {nullptr};
     bool haveEvents = false;
     float kernelUs[8] = {0};
-    int k5Blocks = 0, k6Blocks = 0;
+    int k4Blocks = 0, k5Blocks = 0, k6Blocks = 0;
     size_t k5GridSmem = 0; bool k5SmemGrid = false;
 };
 
@@ -99,6 +99,8 @@ Layout make_layout(const tpc_tracker* t, int64_t maxClusters) {
     L.linkDnC = take(sizeof(int32_t) * L.hitCap);
     L.weight = take(sizeof(uint32_t) * L.hitCap);
     L.starts = take(sizeof(int4) * L.maxTracklets);
+    L.startsRaw = take(sizeof(int4) * L.maxTracklets);
+    L.rowHist = take(sizeof(uint32_t) * 2 * (kMaxRows + 1));
     L.recs = take(sizeof(TrackletRec) * L.maxTracklets);
     L.rowHit = take(sizeof(int32_t) * L.maxTracklets * t->rhStride);
     L.tracks = take(sizeof(tpc_track) * L.maxTracklets);
@@ -118,7 +120,7 @@ void bind_pointers(tpc_tracker* t) {
     d.hits = (float2*)(w + L.hits); d.orig = (uint32_t*)(w + L.orig); d.binStart = (uint32_t*)(w + L.binStart); d.buckets = (Bucket*)(w + L.buckets);
     d.linkUp = (int32_t*)(w + L.linkUp); d.linkDn = (int32_t*)(w + L.linkDn);
     d.linkUpC = (int32_t*)(w + L.linkUpC); d.linkDnC = (int32_t*)(w + L.linkDnC);
-    d.weight = (uint32_t*)(w + L.weight); d.starts = (int4*)(w + L.starts);
+    d.weight = (uint32_t*)(w + L.weight); d.starts = (int4*)(w + L.starts); d.startsRaw = (int4*)(w + L.startsRaw); d.rowHist = (uint32_t*)(w + L.rowHist);
     d.recs = (TrackletRec*)(w + L.recs); d.rowHit = (int32_t*)(w + L.rowHit);
     d.tracks = (tpc_track*)(w + L.tracks); d.clusterIds = (uint32_t*)(w + L.clusterIds);
     d.counters = (uint32_t*)(w + L.counters); d.sectorGidBase = (uint32_t*)(w + L.sectorGidBase);
@@ -280,7 +282,7 @@ __global__ void dump_links_kernel(DevPtrs d, int nRows, int64_t N, int32_t* out)
 __global__ void dump_starts_kernel(DevPtrs d, unsigned n, uint32_t* out) {
     const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    const int4 s = d.starts[i];
+    const int4 s = d.startsRaw[i];      // append order (the row-ordered copy exists only for the phased K5 kernel)
     out[i] = d.orig[d.grid[s.x].hitOff + s.y];
 }
 __global__ void dump_rowhit_kernel(DevPtrs d, int nRows, unsigned n, int32_t* out) {
@@ -398,14 +400,14 @@ int tpc_set_workspace(tpc_tracker* t, void* dev_ptr, size_t bytes) {
         t->k5GridSmem = sizeof(RowGrid) * (size_t)t->nRowsTotal;
         t->k5SmemGrid = t->k5GridSmem + 2048 <= 227 * 1024;
         if (t->k5SmemGrid) {
-            CUDA_TRY(t, cudaFuncSetAttribute(k5_construct<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->k5GridSmem));
-            CUDA_TRY(t, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ5, k5_construct<true>, kK5Threads, t->k5GridSmem));
-        } else {
-            CUDA_TRY(t, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ5, k5_construct<false>, kK5Threads, 0));
+            CUDA_TRY(t, cudaFuncSetAttribute(k5_construct_free<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->k5GridSmem));
+            CUDA_TRY(t, cudaFuncSetAttribute(k5_construct_phased<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->k5GridSmem));
         }
+        occ5 = 1;   // one persistent block per SM (both instantiations must see the same grid)
         CUDA_TRY(t, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ6, k6_select, kK6Threads, 0));
         t->k5Blocks = sms * std::max(1, occ5);
         t->k6Blocks = sms * std::max(1, occ6);
+        t->k4Blocks = sms;
     }
     return tpc_reset_event(t);
 }
@@ -468,13 +470,19 @@ int tpc_track_sectors(tpc_tracker* t) {
     k2_neighbours<<<NR, kK2Threads, 0, s>>>(d, dp);
     CUDA_TRY(t, cudaEventRecord(t->ev[2], s));
     k3_clean_start<<<NR, kK3Threads, 0, s>>>(d, dp);
+    k4_sort_starts<<<t->k5Blocks, kK4Threads, 0, s>>>(d, dp, kK5PhasedThreads / 32);    // same grid as K5: same decision
     CUDA_TRY(t, cudaEventRecord(t->ev[3], s));
     {
-        // enough threads for the tracklet capacity, at most what is resident at once (persistent threads + queue)
-        const int64_t want = (t->L.maxTracklets + kK5Threads - 1) / kK5Threads;
-        const int blocks = (int)std::max<int64_t>(1, std::min<int64_t>(want, t->k5Blocks));
-        if (t->k5SmemGrid) k5_construct<true><<<blocks, kK5Threads, t->k5GridSmem, s>>>(d, dp);
-        else k5_construct<false><<<blocks, kK5Threads, 0, s>>>(d, dp);
+        // one persistent block per SM; the phased and the free-running instantiation decide on the device (from the
+        // number of start hits) which of them does the event, the other returns at once
+        const int blocks = t->k5Blocks;
+        if (t->k5SmemGrid) {
+            k5_construct_phased<true><<<blocks, kK5PhasedThreads, t->k5GridSmem, s>>>(d, dp);
+            k5_construct_free<true><<<blocks, kK5Threads, t->k5GridSmem, s>>>(d, dp, kK5PhasedThreads / 32);
+        } else {
+            k5_construct_phased<false><<<blocks, kK5PhasedThreads, 0, s>>>(d, dp);
+            k5_construct_free<false><<<blocks, kK5Threads, 0, s>>>(d, dp, kK5PhasedThreads / 32);
+        }
     }
     CUDA_TRY(t, cudaEventRecord(t->ev[4], s));
     k6_weights<<<t->k6Blocks, kK6Threads, 0, s>>>(d, dp);
@@ -486,7 +494,7 @@ int tpc_track_sectors(tpc_tracker* t) {
     return TPC_OK;
 }
 
-int tpc_launches_per_track(const tpc_tracker* t) { (void)t; return 6; }
+int tpc_launches_per_track(const tpc_tracker* t) { (void)t; return 8; }
 
 int tpc_sync(tpc_tracker* t) {
     if (!t) return TPC_E_ARG;
