@@ -78,9 +78,12 @@ struct DevPtrs {
     int32_t* linkDnC;
     uint32_t* weight;      // ownership key per hit
     int4* startsRaw;       // K3/K4 output in append order: (rowId, sorted position, sorted position of the linked hit in the
-                           // row above, global id)
-    int4* starts;          // the same, ordered by pad row of the start hit (k4_sort_starts): K5's input
-    uint32_t* rowHist;     // [2][kMaxRows + 1]: start hits per pad row, scatter cursors
+                           // row above, global id); read by the free-running K5 kernel
+    int4* starts;          // the same records filed by pad row: row r's start hits at starts[rowStartBase[r] + 0..rowHist[r]);
+                           // read by the phased K5 kernel, which wants a warp's tracklets to start in the same row
+    uint32_t* rowHist;     // [kMaxRows + 1] start hits per pad row (K3/K4 atomics)
+    const uint32_t* rowStartBase;   // [kMaxRows + 2] host: exclusive prefix over rows of the clusters per row (all sectors) =
+                                    // where row r's segment of starts[] begins (a row has at most as many start hits as hits)
     TrackletRec* recs;
     int32_t* rowHit;       // [maxTracklets][rhStride], GLOBAL sorted position (row hitOff + position) of the tracklet's hit
                            // in each row, -1 none: indexes weight[] / orig[] directly

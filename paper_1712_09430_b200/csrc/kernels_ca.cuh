@@ -30,7 +30,7 @@ __global__ void __launch_bounds__(kK1Threads) k1_sort_grid(DevPtrs d) {
     const int rowId = blockIdx.x;
     const int tid = threadIdx.x;
     if (rowId == 0 && tid < kNCounters) d.counters[tid] = 0u;
-    if (rowId == 0) for (int i = tid; i < 2 * (kMaxRows + 1); i += kK1Threads) d.rowHist[i] = 0u;
+    if (rowId == 0) for (int i = tid; i <= kMaxRows; i += kK1Threads) d.rowHist[i] = 0u;
     const RowMeta M = d.meta[rowId];
     RowGrid R = d.grid[rowId];
     const int n = M.n;
@@ -385,50 +385,19 @@ __global__ void __launch_bounds__(kK3Threads) k3_clean_start(DevPtrs d, DevParam
             const bool stored = isStart && pos < (unsigned)d.maxTracklets;
             if (stored)   // (row, hit, linked hit, canonical id): all K5 needs to begin
                 d.startsRaw[pos] = make_int4(rowId, i, upKeep, (int)d.orig[hitOff + i]);
+            // ... and the same record filed under its pad row (for the phased K5 kernel)
             const unsigned ms = __ballot_sync(0xffffffffu, stored);
-            if (lane == 0 && ms) atomicAdd(&d.rowHist[r], (unsigned)__popc(ms));     // for k4_sort_starts
+            if (ms) {
+                unsigned pr = 0;
+                if (lane == 0) pr = atomicAdd(&d.rowHist[r], (unsigned)__popc(ms));
+                pr = __shfl_sync(0xffffffffu, pr, 0) + __popc(ms & ((1u << lane) - 1u));
+                if (stored) d.starts[d.rowStartBase[r] + pr] = make_int4(rowId, i, upKeep, (int)d.orig[hitOff + i]);
+            }
         }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) nLinks += __shfl_xor_sync(0xffffffffu, nLinks, o);
     if (lane == 0 && nLinks) atomicAdd(&d.counters[kNLinks], nLinks);
-}
-
-// ------------------------------------------------------------------------------------------ K4b
-// Order the start hits by their pad row (counting sort over the row histogram K3/K4 filled).  K5 hands 32 consecutive
-// start hits to a warp and, when there is about one tracklet per thread, takes a warp's tracklets through their legs
-// in phases; that only pays if the tracklets of a warp start in (nearly) the same row, so that their outward legs and
-// their inward extensions have similar lengths.  The order inside a row is arbitrary; no result depends on it
-// (tracklets are identified by the global id of their start hit).
-constexpr int kK4Threads = 256;
-
-__global__ void __launch_bounds__(kK4Threads) k4_sort_starts(DevPtrs d, DevParams dp, int phasedWarps) {
-    __shared__ uint32_t base[kMaxRows + 1];
-    __shared__ uint32_t wsum[kK4Threads / 32];
-    const unsigned n = min(d.counters[kNStart], (unsigned)d.maxTracklets);
-    // only the phased K5 kernel reads the ordered list (same criterion as k5_phased_mode in kernels_kf.cuh)
-    if ((float)n / (32.0f * (float)gridDim.x) > (float)phasedWarps) return;
-    // exclusive prefix sum of the row histogram (n_rows <= 255 < block size): one value per thread
-    const unsigned tid = threadIdx.x, lane = tid & 31u;
-    const uint32_t h = (int)tid < dp.nRows ? d.rowHist[tid] : 0u;
-    uint32_t incl = h;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
-        if (lane >= (unsigned)o) incl += v;
-    }
-    if (lane == 31) wsum[tid >> 5] = incl;
-    __syncthreads();
-    uint32_t off = 0;
-    for (unsigned w = 0; w < (tid >> 5); w++) off += wsum[w];
-    if (tid <= kMaxRows) base[tid] = off + incl - h;
-    __syncthreads();
-    uint32_t* cursor = d.rowHist + (kMaxRows + 1);
-    for (unsigned i = blockIdx.x * kK4Threads + threadIdx.x; i < n; i += gridDim.x * kK4Threads) {
-        const int4 s = d.startsRaw[i];
-        const int r = s.x % dp.nRows;
-        d.starts[base[r] + atomicAdd(&cursor[r], 1u)] = s;
-    }
 }
 
 }  // namespace tpc

@@ -21,7 +21,7 @@ constexpr size_t kAlign = 256;
 inline size_t align_up(size_t v, size_t a = kAlign) { return (v + a - 1) / a * a; }
 
 struct Layout {   // byte offsets into the workspace
-    size_t inY, inZ, grid, meta, rowX, hits, orig, binStart, buckets, linkUp, linkDn, linkUpC, linkDnC, weight, starts, startsRaw, rowHist, recs, rowHit,
+    size_t inY, inZ, grid, meta, rowX, hits, orig, binStart, buckets, linkUp, linkDn, linkUpC, linkDnC, weight, starts, startsRaw, rowHist, rowStartBase, recs, rowHit,
         tracks, clusterIds, counters, sectorGidBase, total;
     int64_t hitCap, binCap, maxTracklets;
 };
@@ -55,6 +55,7 @@ struct tpc_tracker {
     RowMeta* hostMeta = nullptr;            // pinned
     uint32_t* hostSectorBase = nullptr;     // pinned
     uint32_t* hostCounters = nullptr;       // pinned
+    uint32_t* hostRowStartBase = nullptr;   // pinned
     int maxBinsLaunch = 1;
 
     // results (pinned)
@@ -64,7 +65,7 @@ struct tpc_tracker {
     cudaEvent_t ev[8] = {nullptr};
     bool haveEvents = false;
     float kernelUs[8] = {0};
-    int k4Blocks = 0, k5Blocks = 0, k6Blocks = 0;
+    int k5Blocks = 0, k6Blocks = 0;
     size_t k5GridSmem = 0; bool k5SmemGrid = false;
 };
 
@@ -98,9 +99,10 @@ Layout make_layout(const tpc_tracker* t, int64_t maxClusters) {
     L.linkUpC = take(sizeof(int32_t) * L.hitCap);
     L.linkDnC = take(sizeof(int32_t) * L.hitCap);
     L.weight = take(sizeof(uint32_t) * L.hitCap);
-    L.starts = take(sizeof(int4) * L.maxTracklets);
+    L.starts = take(sizeof(int4) * (maxClusters + 16));      // filed by pad row: a row's segment holds as many records as the row has clusters
     L.startsRaw = take(sizeof(int4) * L.maxTracklets);
-    L.rowHist = take(sizeof(uint32_t) * 2 * (kMaxRows + 1));
+    L.rowHist = take(sizeof(uint32_t) * (kMaxRows + 1));
+    L.rowStartBase = take(sizeof(uint32_t) * (kMaxRows + 2));
     L.recs = take(sizeof(TrackletRec) * L.maxTracklets);
     L.rowHit = take(sizeof(int32_t) * L.maxTracklets * t->rhStride);
     L.tracks = take(sizeof(tpc_track) * L.maxTracklets);
@@ -120,7 +122,7 @@ void bind_pointers(tpc_tracker* t) {
     d.hits = (float2*)(w + L.hits); d.orig = (uint32_t*)(w + L.orig); d.binStart = (uint32_t*)(w + L.binStart); d.buckets = (Bucket*)(w + L.buckets);
     d.linkUp = (int32_t*)(w + L.linkUp); d.linkDn = (int32_t*)(w + L.linkDn);
     d.linkUpC = (int32_t*)(w + L.linkUpC); d.linkDnC = (int32_t*)(w + L.linkDnC);
-    d.weight = (uint32_t*)(w + L.weight); d.starts = (int4*)(w + L.starts); d.startsRaw = (int4*)(w + L.startsRaw); d.rowHist = (uint32_t*)(w + L.rowHist);
+    d.weight = (uint32_t*)(w + L.weight); d.starts = (int4*)(w + L.starts); d.startsRaw = (int4*)(w + L.startsRaw); d.rowHist = (uint32_t*)(w + L.rowHist); d.rowStartBase = (const uint32_t*)(w + L.rowStartBase);
     d.recs = (TrackletRec*)(w + L.recs); d.rowHit = (int32_t*)(w + L.rowHit);
     d.tracks = (tpc_track*)(w + L.tracks); d.clusterIds = (uint32_t*)(w + L.clusterIds);
     d.counters = (uint32_t*)(w + L.counters); d.sectorGidBase = (uint32_t*)(w + L.sectorGidBase);
@@ -183,6 +185,7 @@ int finalize_event(tpc_tracker* t) {
         CUDA_TRY(t, cudaMallocHost(&t->hostMeta, sizeof(RowMeta) * (NR + 2)));
         CUDA_TRY(t, cudaMallocHost(&t->hostSectorBase, sizeof(uint32_t) * (t->nSec + 1)));
         CUDA_TRY(t, cudaMallocHost(&t->hostCounters, sizeof(uint32_t) * kNCounters));
+        CUDA_TRY(t, cudaMallocHost(&t->hostRowStartBase, sizeof(uint32_t) * (kMaxRows + 2)));
     } else {
         CUDA_TRY(t, cudaStreamSynchronize(t->stream));   // a previous async upload may still read the host tables
     }
@@ -203,6 +206,13 @@ int finalize_event(tpc_tracker* t) {
         binOff += M.maxBins + 1;
     }
     t->hostSectorBase[t->nSec] = (uint32_t)gid;
+    {   // where each pad row's segment of the by-row start list begins: prefix over rows of the clusters per row
+        uint64_t run = 0;
+        for (int r = 0; r <= t->nRows; r++) {
+            t->hostRowStartBase[r] = (uint32_t)run;
+            if (r < t->nRows) for (int sct = 0; sct < t->nSec; sct++) run += (uint64_t)t->rowN[sct * t->nRows + r];
+        }
+    }
     for (int s = 0; s < t->nSec; s++)
         if ((int64_t)t->hostSectorBase[s + 1] - (int64_t)t->hostSectorBase[s] > 0x00FFFFFF) return TPC_E_ARG;  // key field
     t->nClusters = gid;
@@ -211,6 +221,8 @@ int finalize_event(tpc_tracker* t) {
     CUDA_TRY(t, cudaMemcpyAsync(t->dev.grid, t->hostGrid, sizeof(RowGrid) * NR, cudaMemcpyHostToDevice, t->stream));
     CUDA_TRY(t, cudaMemcpyAsync((void*)t->dev.meta, t->hostMeta, sizeof(RowMeta) * NR, cudaMemcpyHostToDevice, t->stream));
     CUDA_TRY(t, cudaMemcpyAsync(t->dev.sectorGidBase, t->hostSectorBase, sizeof(uint32_t) * (t->nSec + 1),
+                                cudaMemcpyHostToDevice, t->stream));
+    CUDA_TRY(t, cudaMemcpyAsync((void*)t->dev.rowStartBase, t->hostRowStartBase, sizeof(uint32_t) * (t->nRows + 1),
                                 cudaMemcpyHostToDevice, t->stream));
     {
         int rc = flush_dirty(t);
@@ -356,6 +368,7 @@ void tpc_tracker_destroy(tpc_tracker* t) {
     if (t->hostMeta) cudaFreeHost(t->hostMeta);
     if (t->hostSectorBase) cudaFreeHost(t->hostSectorBase);
     if (t->hostCounters) cudaFreeHost(t->hostCounters);
+    if (t->hostRowStartBase) cudaFreeHost(t->hostRowStartBase);
     if (t->outTracks) cudaFreeHost(t->outTracks);
     if (t->outIds) cudaFreeHost(t->outIds);
     if (t->haveEvents) for (auto& e : t->ev) cudaEventDestroy(e);
@@ -407,7 +420,6 @@ int tpc_set_workspace(tpc_tracker* t, void* dev_ptr, size_t bytes) {
         CUDA_TRY(t, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ6, k6_select, kK6Threads, 0));
         t->k5Blocks = sms * std::max(1, occ5);
         t->k6Blocks = sms * std::max(1, occ6);
-        t->k4Blocks = sms;
     }
     return tpc_reset_event(t);
 }
@@ -470,7 +482,6 @@ int tpc_track_sectors(tpc_tracker* t) {
     k2_neighbours<<<NR, kK2Threads, 0, s>>>(d, dp);
     CUDA_TRY(t, cudaEventRecord(t->ev[2], s));
     k3_clean_start<<<NR, kK3Threads, 0, s>>>(d, dp);
-    k4_sort_starts<<<t->k5Blocks, kK4Threads, 0, s>>>(d, dp, kK5PhasedThreads / 32);    // same grid as K5: same decision
     CUDA_TRY(t, cudaEventRecord(t->ev[3], s));
     {
         // one persistent block per SM; the phased and the free-running instantiation decide on the device (from the
@@ -494,7 +505,7 @@ int tpc_track_sectors(tpc_tracker* t) {
     return TPC_OK;
 }
 
-int tpc_launches_per_track(const tpc_tracker* t) { (void)t; return 8; }
+int tpc_launches_per_track(const tpc_tracker* t) { (void)t; return 7; }
 
 int tpc_sync(tpc_tracker* t) {
     if (!t) return TPC_E_ARG;
