@@ -331,11 +331,11 @@ def main():
     value, ms, n_total = aggregate(dist, dev, ev.n_clusters, step_ms)
 
     # ---- end to end through the C ABI with HOST buffers (pinned), H2D + D2H of every step inside the timed region.
-    # Three tracker instances, each driven by its own host thread on its own stream, take events in turn: while one
+    # Four tracker instances, each driven by its own host thread on its own stream, take events in turn: while one
     # tracks, the others upload their next event / download their tracks (the paper's DMA || kernel pipeline,
     # PAPER.md:66 and Fig. 4).  Every step still does load_event (pinned host -> device), track_sectors, get_tracks
     # (device -> pinned host); time = wall clock around all steps of both threads.
-    n_pipe = 3      # measured on config 3: 2 / 3 / 4 instances -> 0.99 / 0.76 / 0.84 ms per event
+    n_pipe = 4      # measured on config 3, two boxes: 2 / 3 / 4 instances -> 0.99 / 0.76 / 0.84 and 1.25 / 1.03 / 0.78 ms per event
     pipes = []
     for i in range(n_pipe):
         sti = torch.cuda.Stream(device=dev)
@@ -367,7 +367,7 @@ def main():
     e2e_run(2)
     if dist is not None:
         dist.barrier()
-    n_e2e = max(4, min(args.steps, 20)) // n_pipe * n_pipe
+    n_e2e = max(8, min(args.steps, 24)) // n_pipe * n_pipe
     e2e_ms = e2e_run(n_e2e // n_pipe) / n_e2e * 1e3
     tr, ids = last[0]
     e2e_value, e2e_ms_max, _ = aggregate(dist, dev, ev.n_clusters, e2e_ms)
@@ -400,7 +400,7 @@ def main():
                    "grid_bins_per_hit": float(params.grid_bins_per_hit)},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms_max, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "steps": n_e2e, "pipeline": "3 tracker instances / host threads / streams: copies of one event overlap the kernels of the others"},
+                "steps": n_e2e, "pipeline": "4 tracker instances / host threads / streams: copies of one event overlap the kernels of the others"},
         "gpu_launches": args.steps * trk.launches_per_track(),
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": round(achieved, 2), "peak": peak, "unit": "GB/s",
                      "frac": round(achieved / peak, 5), "traffic": traffic, "peak_source": peak_src,
