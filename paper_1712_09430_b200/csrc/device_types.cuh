@@ -49,7 +49,8 @@ struct __align__(16) TrackletRec {
     float p[5];
     float c[15];
     float chi2;
-    float pad[3];
+    uint32_t ownerKey;     // K6's ownership key (S6), written by K5 with the record
+    float pad[2];
 };
 static_assert(sizeof(TrackletRec) == 128, "TrackletRec layout");
 
@@ -59,7 +60,7 @@ struct DevParams {
     int32_t nSec, nRows;
 };
 
-enum Counter { kNStart = 0, kQueue = 1, kNTracks = 2, kNTrackClusters = 3, kNKept = 4, kHitsTotal = 5, kNLinks = 6, kNCounters = 16 };
+enum Counter { kNStart = 0, kQueue = 1, kNTracks = 2, kNTrackClusters = 3 /* = kNTracks + 1, 8-byte aligned pair (K6b) */, kNKept = 4, kHitsTotal = 5, kNLinks = 6, kNCounters = 16 };
 
 // All device pointers of one tracker; passed by value to the kernels.
 struct DevPtrs {

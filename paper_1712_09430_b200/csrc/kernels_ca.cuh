@@ -329,7 +329,7 @@ __global__ void __launch_bounds__(kK2Threads, TPC_K2B) k2_neighbours(DevPtrs d, 
 // ------------------------------------------------------------------------------------------ K3 + K4
 // Cleaner (S3): keep reciprocal links only.  Start hits (S4): no down-link, chain of >= seed_min_chain hits.
 // The chain test re-derives the cleaned up-links of the next rows from the raw links (same predicate), so one
-// kernel does both; the start list is appended with one atomic per warp (ballot + prefix).
+// kernel does both; the start lists are appended with one atomic per block (collected in shared memory).
 #ifndef TPC_K3T
 #define TPC_K3T 64
 #endif
@@ -340,6 +340,9 @@ __device__ __forceinline__ int clean_up_link(const DevPtrs& d, int hitOff, int h
     return (u >= 0 && d.linkDn[hitOffUp + u] == i) ? u : -1;
 }
 
+constexpr int kK3Buf = 512;    // start hits a block collects in shared memory before it appends them (8 KB)
+static_assert(kK3Buf % kK3Threads == 0, "K3 empties its buffer on iteration boundaries");
+
 __global__ void __launch_bounds__(kK3Threads) k3_clean_start(DevPtrs d, DevParams dp) {
     // Blocks run pad row by pad row (all sectors of row 0, then row 1, ...): blocks are dispatched in index order, so
     // the start list comes out roughly ordered by pad row.  K5 gives 32 consecutive start hits to a warp; tracklets
@@ -349,6 +352,34 @@ __global__ void __launch_bounds__(kK3Threads) k3_clean_start(DevPtrs d, DevParam
     const int rowId = (blockIdx.x - r * dp.nSec) * dp.nRows + r;
     const int n = d.meta[rowId].n;
     if (n == 0) return;
+    // The block's start hits are collected in shared memory and appended with ONE atomic per list and block: with
+    // an atomic per warp and 64 hits, half of the kernel's time was spent waiting in line at counters[kNStart].
+    __shared__ int4 sStart[kK3Buf];
+    __shared__ unsigned sCount, sBaseRaw, sBaseRow, sStored;
+    if (threadIdx.x == 0) sCount = 0u;
+    __syncthreads();
+    auto flush = [&]() {      // called by all threads
+        __syncthreads();
+        const unsigned cnt = sCount;
+        if (cnt == 0u) return;
+        if (threadIdx.x == 0) {
+            const unsigned raw = atomicAdd(&d.counters[kNStart], cnt);
+            const unsigned room = raw < (unsigned)d.maxTracklets ? (unsigned)d.maxTracklets - raw : 0u;
+            const unsigned nst = min(cnt, room);
+            sBaseRaw = raw; sStored = nst;
+            sBaseRow = nst ? atomicAdd(&d.rowHist[r], nst) : 0u;     // ... and filed under its pad row (phased K5)
+        }
+        __syncthreads();
+        const unsigned nst = sStored, b0 = sBaseRaw, b1 = d.rowStartBase[r] + sBaseRow;
+        for (unsigned k = threadIdx.x; k < nst; k += kK3Threads) {
+            const int4 v = sStart[k];
+            d.startsRaw[b0 + k] = v;
+            d.starts[b1 + k] = v;
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) sCount = 0u;
+        __syncthreads();
+    };
     const bool hasUp = r + 1 < dp.nRows, hasDn = r >= 1;
     const int hitOff = d.grid[rowId].hitOff;
     const int hitOffU = hasUp ? d.grid[rowId + 1].hitOff : hitOff;
@@ -377,24 +408,18 @@ __global__ void __launch_bounds__(kK3Threads) k3_clean_start(DevPtrs d, DevParam
                 isStart = len >= dp.P.seed_min_chain;
             }
         }
+        // rows with more hits than the buffer holds empty it every kK3Buf hits (uniform: base is the block's)
+        if (base > 0 && base % kK3Buf == 0) flush();
         const unsigned m = __ballot_sync(0xffffffffu, isStart);
         if (m) {
             unsigned pos = 0;
-            if (lane == 0) pos = atomicAdd(&d.counters[kNStart], (unsigned)__popc(m));
+            if (lane == 0) pos = atomicAdd(&sCount, (unsigned)__popc(m));
             pos = __shfl_sync(0xffffffffu, pos, 0) + __popc(m & ((1u << lane) - 1u));
-            const bool stored = isStart && pos < (unsigned)d.maxTracklets;
-            if (stored)   // (row, hit, linked hit, canonical id): all K5 needs to begin
-                d.startsRaw[pos] = make_int4(rowId, i, upKeep, (int)d.orig[hitOff + i]);
-            // ... and the same record filed under its pad row (for the phased K5 kernel)
-            const unsigned ms = __ballot_sync(0xffffffffu, stored);
-            if (ms) {
-                unsigned pr = 0;
-                if (lane == 0) pr = atomicAdd(&d.rowHist[r], (unsigned)__popc(ms));
-                pr = __shfl_sync(0xffffffffu, pr, 0) + __popc(ms & ((1u << lane) - 1u));
-                if (stored) d.starts[d.rowStartBase[r] + pr] = make_int4(rowId, i, upKeep, (int)d.orig[hitOff + i]);
-            }
+            if (isStart)   // (row, hit, linked hit, canonical id): all K5 needs to begin
+                sStart[pos] = make_int4(rowId, i, upKeep, (int)d.orig[hitOff + i]);
         }
     }
+    flush();
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) nLinks += __shfl_xor_sync(0xffffffffu, nLinks, o);
     if (lane == 0 && nLinks) atomicAdd(&d.counters[kNLinks], nLinks);

@@ -65,7 +65,7 @@ struct tpc_tracker {
     cudaEvent_t ev[8] = {nullptr};
     bool haveEvents = false;
     float kernelUs[8] = {0};
-    int k5Blocks = 0, k6Blocks = 0;
+    int k5Blocks = 0, k6Blocks = 0, k6aBlocks = 0;
     size_t k5GridSmem = 0; bool k5SmemGrid = false;
 };
 
@@ -420,6 +420,9 @@ int tpc_set_workspace(tpc_tracker* t, void* dev_ptr, size_t bytes) {
         CUDA_TRY(t, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ6, k6_select, kK6Threads, 0));
         t->k5Blocks = sms * std::max(1, occ5);
         t->k6Blocks = sms * std::max(1, occ6);
+        int occ6a = 0;
+        CUDA_TRY(t, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ6a, k6_weights, kK6Threads, 0));
+        t->k6aBlocks = sms * std::max(1, occ6a);
     }
     return tpc_reset_event(t);
 }
@@ -496,7 +499,7 @@ int tpc_track_sectors(tpc_tracker* t) {
         }
     }
     CUDA_TRY(t, cudaEventRecord(t->ev[4], s));
-    k6_weights<<<t->k6Blocks, kK6Threads, 0, s>>>(d, dp);
+    k6_weights<<<t->k6aBlocks, kK6Threads, 0, s>>>(d, dp);
     CUDA_TRY(t, cudaEventRecord(t->ev[5], s));
     k6_select<<<2 * t->k6Blocks, kK6Threads, 0, s>>>(d, dp);   // measured: 2 waves of warps beat 1 here (45 vs 50 us), not in K6a
     CUDA_TRY(t, cudaEventRecord(t->ev[6], s));
