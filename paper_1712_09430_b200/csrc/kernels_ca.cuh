@@ -226,9 +226,21 @@ __device__ __forceinline__ void scan_ranges(const WinRanges& w, const RowGrid& R
                                             const uint32_t* __restrict__ binStart, F&& f) {
     const float2* __restrict__ hs = hits + R.hitOff;
     if (w.bz1 - w.bz0 <= 2) {
-#pragma unroll
-        for (int j = 0; j < 3; j++)
-            for (int k = w.k0[j]; k < w.k1[j]; k++) f(k, hs[k]);
+        // one loop over the three ranges laid end to end: the warp runs max over lanes of the TOTAL length, not the
+        // sum over ranges of the per-range maxima
+        const int l0 = w.k1[0] - w.k0[0], l1 = l0 + (w.k1[1] - w.k0[1]), l2 = l1 + (w.k1[2] - w.k0[2]);
+        const int o1 = w.k0[1] - l0, o2 = w.k0[2] - l1;
+        auto at = [&](int t) { return t < l0 ? w.k0[0] + t : t < l1 ? o1 + t : o2 + t; };
+        if (l2 > 0) {
+            int k = at(0);
+            float2 c = hs[k];
+            for (int t = 0; t < l2; t++) {
+                const int kn = at(min(t + 1, l2 - 1));      // next candidate requested before this one is examined
+                const float2 cn = hs[kn];
+                f(k, c);
+                k = kn; c = cn;
+            }
+        }
     } else {
         const uint32_t* __restrict__ bs = binStart + R.binOff;
         for (int bz = w.bz0; bz <= w.bz1; bz++) {
