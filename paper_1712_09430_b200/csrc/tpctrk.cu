@@ -333,7 +333,7 @@ void tpc_default_params(tpc_params* p) {
     p->road_nsig = 4.0f; p->road_max = 2.0f;
     p->max_gap = 4; p->min_hits = 10; p->seed_min_chain = 3;
     p->max_tracklets_per_cluster = 0.125f;
-    p->grid_bins_per_hit = 4.0f;
+    p->grid_bins_per_hit = 3.0f;
 }
 
 int tpc_tracker_create(const tpc_geometry* g, float bz_tesla, tpc_tracker** out) {
