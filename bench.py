@@ -259,6 +259,7 @@ def main():
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--e2e-instances", type=int, default=4, help="tracker instances / host threads / streams of the end-to-end leg")
     ap.add_argument("--bins-per-hit", type=float, default=None, help="override tpc_params.grid_bins_per_hit (tuning)")
     ap.add_argument("--events-per-call", type=int, default=4,
                     help="extra leg: this many events tracked by one call (PAPER.md:82-84); 0 or 1 = skip")
@@ -335,7 +336,7 @@ def main():
     # tracks, the others upload their next event / download their tracks (the paper's DMA || kernel pipeline,
     # PAPER.md:66 and Fig. 4).  Every step still does load_event (pinned host -> device), track_sectors, get_tracks
     # (device -> pinned host); time = wall clock around all steps of both threads.
-    n_pipe = 4      # measured on config 3, two boxes: 2 / 3 / 4 instances -> 0.99 / 0.76 / 0.84 and 1.25 / 1.03 / 0.78 ms per event
+    n_pipe = max(1, args.e2e_instances)      # measured on config 3, two boxes: 2 / 3 / 4 instances -> 0.99 / 0.76 / 0.84 and 1.25 / 1.03 / 0.78 ms per event
     pipes = []
     for i in range(n_pipe):
         sti = torch.cuda.Stream(device=dev)
