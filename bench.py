@@ -378,6 +378,10 @@ def main():
     # ---- roofline of the dominant kernel + per-kernel table
     peak, peak_src = measured_peaks()
     ab = algorithmic_bytes(st)
+    if st.get("k6a_fused"):
+        # the phased K5 kernel ran the K6a weights pass itself: its bytes are K5's, K6a's launch returned at once
+        ab["K5_construct"] += ab["K6a_weights"]
+        ab["K6a_weights"] = 0
     dom = max(kern, key=kern.get)
     per_kernel = {k: {"us": round(kern[k], 2), "alg_bytes": ab[k], "gbs": round(ab[k] / (kern[k] * 1e-6) / 1e9, 1),
                       "frac": round(ab[k] / (kern[k] * 1e-6) / 1e9 / peak, 4)} for k in kern}
@@ -398,7 +402,8 @@ def main():
                    "parallelism": "one event per GPU, no collective" if world > 1 else "single GPU",
                    "n_start_hits": st["n_start_hits"], "n_tracklet_hits": st["n_tracklet_hits"], "n_tracks": st["n_tracks"],
                    "workspace_bytes": ws_bytes, "workspace_over_input": round(ws_bytes / (12.0 * ev.n_clusters), 2),
-                   "grid_bins_per_hit": float(params.grid_bins_per_hit)},
+                   "grid_bins_per_hit": float(params.grid_bins_per_hit),
+                   "k6a_fused_into_k5": bool(st.get("k6a_fused"))},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms_max, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "steps": n_e2e, "pipeline": "4 tracker instances / host threads / streams: copies of one event overlap the kernels of the others"},

@@ -86,7 +86,9 @@ typedef struct tpc_stats {
     int64_t n_clusters, n_links, n_start_hits, n_tracklets, n_tracklet_hits, n_tracks, n_track_clusters;
     int64_t workspace_bytes_used, max_clusters, max_tracklets;
     float kernel_us[8];       /* K1 sort+grid, K2 neighbours, K3/K4 clean+start, K5 construct, K6a weights,
-                                 K6b select+compact, [6] = K1..K6 total, [7] = unused */
+                                 K6b select+compact, [6] = K1..K6 total, [7] = 1.0 if the K6a weights pass of this
+                                 event ran inside the K5 launch (about one tracklet per GPU thread or fewer: [3]
+                                 then includes it and [4] is a launch that returns at once), else 0.0 */
 } tpc_stats;
 
 /* Record of tpc_debug_dump(TPC_DUMP_TRACKLETS). */

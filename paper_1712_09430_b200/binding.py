@@ -220,6 +220,7 @@ class Tracker:
         d = {k: int(getattr(s, k)) for k, _ in tpc_stats._fields_ if k != "kernel_us"}
         d["kernel_us"] = dict(zip(KERNEL_NAMES, [float(v) for v in s.kernel_us[:6]]))
         d["total_us"] = float(s.kernel_us[6])
+        d["k6a_fused"] = bool(s.kernel_us[7] > 0.5)
         return d
 
     def launches_per_track(self) -> int:

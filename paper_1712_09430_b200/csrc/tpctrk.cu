@@ -499,7 +499,7 @@ int tpc_track_sectors(tpc_tracker* t) {
         }
     }
     CUDA_TRY(t, cudaEventRecord(t->ev[4], s));
-    k6_weights<<<t->k6aBlocks, kK6Threads, 0, s>>>(d, dp);
+    k6_weights<<<t->k6aBlocks, kK6Threads, 0, s>>>(d, dp, t->k5Blocks);
     CUDA_TRY(t, cudaEventRecord(t->ev[5], s));
     k6_select<<<2 * t->k6Blocks, kK6Threads, 0, s>>>(d, dp);   // measured: 2 waves of warps beat 1 here (45 vs 50 us), not in K6a
     CUDA_TRY(t, cudaEventRecord(t->ev[6], s));
@@ -523,7 +523,11 @@ int tpc_sync(tpc_tracker* t) {
         t->kernelUs[i] = ms * 1000.f;
     }
     CUDA_TRY(t, cudaEventElapsedTime(&total, t->ev[0], t->ev[6]));
-    t->kernelUs[6] = total * 1000.f; t->kernelUs[7] = 0.f;
+    t->kernelUs[6] = total * 1000.f;
+    // [7]: 1 if this event was the phased K5 kernel's, whose warps run the K6a weights pass themselves (same test as
+    // k5_phased_mode on the device); K6a's own launch then returned at once
+    const unsigned nTotal = (unsigned)std::min<int64_t>(t->counters[kNStart], t->dev.maxTracklets);
+    t->kernelUs[7] = (TPC_K5_FUSE_K6A && (float)nTotal / (32.0f * (float)t->k5Blocks) <= (float)(kK5PhasedThreads / 32)) ? 1.f : 0.f;
     return TPC_OK;
 }
 

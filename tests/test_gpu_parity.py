@@ -35,6 +35,8 @@ def test_configs_match_oracle_stage_by_stage(cfg):
     assert st["n_tracklets"] == int(ref.tracklets["kept"].sum())
     assert st["n_tracklet_hits"] == int(ref.tracklets["n_hits"].sum())
     assert st["n_links"] == int((ref.link_up_clean >= 0).sum())
+    # one event: the phased K5 kernel, whose warps run the K6a weights pass themselves (the counts above come from it)
+    assert st["k6a_fused"]
     # truth metric within 0.1 % of the oracle's
     eg = datagen.efficiency(ev, ids.astype(np.int64), tracks["cluster_offset"], tracks["n_clusters"])
     eo = datagen.efficiency(ev, ref.cluster_ids, ref.tracks["cluster_offset"], ref.tracks["n_clusters"])
@@ -307,6 +309,7 @@ def test_four_central_events_per_call_sampled_sectors():
                        np.concatenate([e.truth for e in evs]))
     trk, tracks, ids = run_gpu(ev)
     assert np.unique(ids).size == ids.size and tracks["n_clusters"].min() >= 10
+    assert not trk.get_stats()["k6a_fused"]          # free-running K5 + the K6a launch
     base = ev.row_base
     for s in (5, 36 + 20, 3 * 36 + 35):
         ref = oracle.run_event(ev.sector_slice(s))
