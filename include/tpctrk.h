@@ -88,7 +88,7 @@ typedef struct tpc_stats {
     float kernel_us[8];       /* K1 sort+grid, K2 neighbours, K3/K4 clean+start, K5 construct, K6a weights,
                                  K6b select+compact, [6] = K1..K6 total, [7] = 1.0 if the K6a weights pass of this
                                  event ran inside the K5 launch (about one tracklet per GPU thread or fewer: [3]
-                                 then includes it and [4] is a launch that returns at once), else 0.0 */
+                                 then includes it and [4] only covers the few tracklets the last K5 warps left over), else 0.0 */
 } tpc_stats;
 
 /* Record of tpc_debug_dump(TPC_DUMP_TRACKLETS). */

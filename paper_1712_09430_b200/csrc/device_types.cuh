@@ -60,7 +60,10 @@ struct DevParams {
     int32_t nSec, nRows;
 };
 
-enum Counter { kNStart = 0, kQueue = 1, kNTracks = 2, kNTrackClusters = 3 /* = kNTracks + 1, 8-byte aligned pair (K6b) */, kNKept = 4, kHitsTotal = 5, kNLinks = 6, kNCounters = 16 };
+enum Counter { kNStart = 0, kQueue = 1, kNTracks = 2, kNTrackClusters = 3 /* = kNTracks + 1, 8-byte aligned pair (K6b) */, kNKept = 4, kHitsTotal = 5, kNLinks = 6, kWarpsDone = 7 /* phased K5: warps that have finished their tracklets */,
+               kNPending = 8 /* ... and how many of them left their K6a weights pass to the k6_weights launch */, kNCounters = 16 };
+// counters[kNCounters + i], i < kMaxPending: the groups of 32 tracklet slots whose weights pass is still to do
+enum : int { kMaxPending = 4096 };
 
 // All device pointers of one tracker; passed by value to the kernels.
 struct DevPtrs {

@@ -107,7 +107,7 @@ Layout make_layout(const tpc_tracker* t, int64_t maxClusters) {
     L.rowHit = take(sizeof(int32_t) * L.maxTracklets * t->rhStride);
     L.tracks = take(sizeof(tpc_track) * L.maxTracklets);
     L.clusterIds = take(sizeof(uint32_t) * (maxClusters + 16));
-    L.counters = take(sizeof(uint32_t) * kNCounters);
+    L.counters = take(sizeof(uint32_t) * (kNCounters + kMaxPending));
     L.sectorGidBase = take(sizeof(uint32_t) * (t->nSec + 1));
     L.total = o;
     return L;
@@ -525,7 +525,7 @@ int tpc_sync(tpc_tracker* t) {
     CUDA_TRY(t, cudaEventElapsedTime(&total, t->ev[0], t->ev[6]));
     t->kernelUs[6] = total * 1000.f;
     // [7]: 1 if this event was the phased K5 kernel's, whose warps run the K6a weights pass themselves (same test as
-    // k5_phased_mode on the device); K6a's own launch then returned at once
+    // k5_phased_mode on the device); K6a's own launch then only did the few groups the last warps left to it
     const unsigned nTotal = (unsigned)std::min<int64_t>(t->counters[kNStart], t->dev.maxTracklets);
     t->kernelUs[7] = (TPC_K5_FUSE_K6A && (float)nTotal / (32.0f * (float)t->k5Blocks) <= (float)(kK5PhasedThreads / 32)) ? 1.f : 0.f;
     return TPC_OK;
