@@ -207,6 +207,10 @@ def multi_event_leg(torch, binding, datagen, args, params, dev, rank: int, k: in
         if i >= 3:
             times.append(a.elapsed_time(b))
     ms = sum(times) / len(times)
+    trk.set_kernel_timing(True)                  # one more call with the events between the kernels, for the table only
+    flush.fill_(1)
+    trk.track_sectors()
+    trk.sync()
     st = trk.get_stats()
     trk.destroy()
     return {"events_per_call": k, "calls": reps, "n_clusters_per_call": n_total, "ms_per_call": ms, "ms_per_event": ms / k,
@@ -315,6 +319,18 @@ def main():
     sampler = ClockSampler(local)
     sampler.start()
     torch.cuda.synchronize()
+    # timed region: K steps as a user runs them (no CUDA events between the kernels: tpctrk.h tpc_set_kernel_timing)
+    events = []
+    for _ in range(args.steps):
+        events.append(step_device())
+        trk.sync()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    step_ms = sum(a.elapsed_time(b) for a, b in events) / args.steps
+    # the same K steps again with an event between the kernels: per-kernel times for the roofline / kernel table
+    # (the five extra event records cost ~14 us per step, reported as ms_per_step_kernel_timing)
+    trk.set_kernel_timing(True)
     events, kern = [], {k: 0.0 for k in binding.KERNEL_NAMES}
     for _ in range(args.steps):
         events.append(step_device())
@@ -323,10 +339,9 @@ def main():
         for k, v in st["kernel_us"].items():
             kern[k] += v
     torch.cuda.synchronize()
-    if dist is not None:
-        dist.barrier()
     clocks = sampler.stop()
-    step_ms = sum(a.elapsed_time(b) for a, b in events) / args.steps
+    step_ms_timing = sum(a.elapsed_time(b) for a, b in events) / args.steps
+    trk.set_kernel_timing(False)
     kern = {k: v / args.steps for k, v in kern.items()}
     st = trk.get_stats()
     value, ms, n_total = aggregate(dist, dev, ev.n_clusters, step_ms)
@@ -403,7 +418,9 @@ def main():
                    "n_start_hits": st["n_start_hits"], "n_tracklet_hits": st["n_tracklet_hits"], "n_tracks": st["n_tracks"],
                    "workspace_bytes": ws_bytes, "workspace_over_input": round(ws_bytes / (12.0 * ev.n_clusters), 2),
                    "grid_bins_per_hit": float(params.grid_bins_per_hit),
-                   "k6a_fused_into_k5": bool(st.get("k6a_fused"))},
+                   "k6a_fused_into_k5": bool(st.get("k6a_fused")),
+                   "ms_per_step_kernel_timing": step_ms_timing,
+                   "kernel_times": "second pass of the same K steps with a CUDA event between the kernels (tpc_set_kernel_timing)"},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms_max, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "steps": n_e2e, "pipeline": "4 tracker instances / host threads / streams: copies of one event overlap the kernels of the others"},

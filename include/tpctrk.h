@@ -117,6 +117,12 @@ void tpc_tracker_destroy(tpc_tracker* t);
 /* cuda_stream: a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = default stream. */
 int tpc_set_stream(tpc_tracker* t, void* cuda_stream);
 
+/* Per-kernel times in tpc_stats.kernel_us[0..5]: on != 0 records a CUDA event between the kernels of every
+ * tpc_track_sectors.  Off by default: the five records keep one kernel's launch from overlapping the end of the
+ * one before it and cost ~14 us per call (2.4 % of a central event).  kernel_us[6] (K1..K6 total) is always
+ * measured; with the timing off kernel_us[0..5] are 0. */
+int tpc_set_kernel_timing(tpc_tracker* t, int on);
+
 /* Device bytes needed for events of up to max_clusters clusters (internal buffers). */
 size_t tpc_workspace_bytes(const tpc_tracker* t, int64_t max_clusters);
 /* dev_ptr: device pointer, 256-byte aligned, caller-owned, must outlive its use.  Capacity is derived from bytes. */

@@ -35,6 +35,7 @@ struct tpc_tracker {
     float bz = 0.f, CB = 0.f;
     cudaStream_t stream = nullptr;
     int lastCuda = 0;
+    bool kernelTiming = false, timedCall = false;   // tpc_set_kernel_timing; whether the last call recorded ev[1..5]
 
     // workspace
     char* ws = nullptr;
@@ -376,6 +377,12 @@ void tpc_tracker_destroy(tpc_tracker* t) {
     delete t;
 }
 
+int tpc_set_kernel_timing(tpc_tracker* t, int on) {
+    if (!t) return TPC_E_ARG;
+    t->kernelTiming = on != 0;
+    return TPC_OK;
+}
+
 int tpc_set_stream(tpc_tracker* t, void* cuda_stream) {
     if (!t) return TPC_E_ARG;
     t->stream = (cudaStream_t)cuda_stream;
@@ -479,13 +486,15 @@ int tpc_track_sectors(tpc_tracker* t) {
     DevParams dp; dp.P = t->P; dp.CB = t->CB; dp.nSec = t->nSec; dp.nRows = t->nRows;
     const int NR = t->nRowsTotal;
     cudaStream_t s = t->stream;
+    const bool timed = t->kernelTiming;     // events between the kernels only on request (tpctrk.h)
+    t->timedCall = timed;
     CUDA_TRY(t, cudaEventRecord(t->ev[0], s));
     k1_sort_grid<<<NR, kK1Threads, sizeof(uint32_t) * (t->maxBinsLaunch + 1), s>>>(d);
-    CUDA_TRY(t, cudaEventRecord(t->ev[1], s));
+    if (timed) CUDA_TRY(t, cudaEventRecord(t->ev[1], s));
     k2_neighbours<<<NR, kK2Threads, 0, s>>>(d, dp);
-    CUDA_TRY(t, cudaEventRecord(t->ev[2], s));
+    if (timed) CUDA_TRY(t, cudaEventRecord(t->ev[2], s));
     k3_clean_start<<<NR, kK3Threads, 0, s>>>(d, dp);
-    CUDA_TRY(t, cudaEventRecord(t->ev[3], s));
+    if (timed) CUDA_TRY(t, cudaEventRecord(t->ev[3], s));
     {
         // one persistent block per SM; the phased and the free-running instantiation decide on the device (from the
         // number of start hits) which of them does the event, the other returns at once
@@ -498,9 +507,9 @@ int tpc_track_sectors(tpc_tracker* t) {
             k5_construct_free<false><<<blocks, kK5Threads, 0, s>>>(d, dp, kK5PhasedThreads / 32);
         }
     }
-    CUDA_TRY(t, cudaEventRecord(t->ev[4], s));
+    if (timed) CUDA_TRY(t, cudaEventRecord(t->ev[4], s));
     k6_weights<<<t->k6aBlocks, kK6Threads, 0, s>>>(d, dp, t->k5Blocks);
-    CUDA_TRY(t, cudaEventRecord(t->ev[5], s));
+    if (timed) CUDA_TRY(t, cudaEventRecord(t->ev[5], s));
     k6_select<<<2 * t->k6Blocks, kK6Threads, 0, s>>>(d, dp);   // measured: 2 waves of warps beat 1 here (45 vs 50 us), not in K6a
     CUDA_TRY(t, cudaEventRecord(t->ev[6], s));
     CUDA_TRY(t, cudaGetLastError());
@@ -519,7 +528,7 @@ int tpc_sync(tpc_tracker* t) {
     float total = 0.f;
     for (int i = 0; i < 6; i++) {
         float ms = 0.f;
-        CUDA_TRY(t, cudaEventElapsedTime(&ms, t->ev[i], t->ev[i + 1]));
+        if (t->timedCall) CUDA_TRY(t, cudaEventElapsedTime(&ms, t->ev[i], t->ev[i + 1]));
         t->kernelUs[i] = ms * 1000.f;
     }
     CUDA_TRY(t, cudaEventElapsedTime(&total, t->ev[0], t->ev[6]));
