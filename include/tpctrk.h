@@ -118,9 +118,10 @@ void tpc_tracker_destroy(tpc_tracker* t);
 int tpc_set_stream(tpc_tracker* t, void* cuda_stream);
 
 /* Per-kernel times in tpc_stats.kernel_us[0..5]: on != 0 records a CUDA event between the kernels of every
- * tpc_track_sectors.  Off by default: the five records keep one kernel's launch from overlapping the end of the
- * one before it and cost ~14 us per call (2.4 % of a central event).  kernel_us[6] (K1..K6 total) is always
- * measured; with the timing off kernel_us[0..5] are 0. */
+ * tpc_track_sectors.  Off by default: without the events K2..K6 are launched as programmatic dependents of the
+ * kernel before them (a kernel's launch, and K5's shared-memory prologue, overlap the end of the previous kernel),
+ * which the event records prevent: ~30 us per call (5 % of a central event).  kernel_us[6] (K1..K6 total) is always
+ * measured; with the timing off kernel_us[0..5] are 0.  Results are identical either way. */
 int tpc_set_kernel_timing(tpc_tracker* t, int on);
 
 /* Device bytes needed for events of up to max_clusters clusters (internal buffers). */

@@ -54,6 +54,17 @@ struct __align__(16) TrackletRec {
 };
 static_assert(sizeof(TrackletRec) == 128, "TrackletRec layout");
 
+// Programmatic dependent launch (tpctrk.cu launches K2..K6 as dependents of the kernel before them when no CUDA events
+// sit between the kernels): grid_dep_wait() returns when the preceding kernel has completed and its writes are
+// visible; every thread of every dependent kernel calls it on every path before it reads anything an earlier kernel
+// of the call wrote and before it exits, so that "this kernel has completed" keeps implying "all earlier ones have".
+// A no-op for a kernel launched the ordinary way.  grid_dep_trigger(): the dependent kernel may start its prologue.
+#ifndef TPC_PDL_TRIGGER
+#define TPC_PDL_TRIGGER 1
+#endif
+__device__ __forceinline__ void grid_dep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void grid_dep_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 struct DevParams {
     tpc_params P;
     float CB;          // curvature per unit q/pT: kappa = p[4]*CB  [1/cm per c/GeV]

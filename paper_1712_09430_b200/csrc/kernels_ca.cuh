@@ -265,6 +265,7 @@ constexpr int kK2Cap = TPC_K2CAP;   // down-candidates cached per thread; beyond
 #define TPC_K2B 8
 #endif
 __global__ void __launch_bounds__(kK2Threads, TPC_K2B) k2_neighbours(DevPtrs d, DevParams dp) {
+    grid_dep_wait();
     const int rowId = blockIdx.x;
     const int r = rowId % dp.nRows;
     const int n = d.meta[rowId].n;
@@ -356,6 +357,10 @@ constexpr int kK3Buf = 512;    // start hits a block collects in shared memory b
 static_assert(kK3Buf % kK3Threads == 0, "K3 empties its buffer on iteration boundaries");
 
 __global__ void __launch_bounds__(kK3Threads) k3_clean_start(DevPtrs d, DevParams dp) {
+    grid_dep_wait();
+#if TPC_PDL_TRIGGER
+    grid_dep_trigger();      // K5 may stage its row table (written by K1) while this kernel runs out
+#endif
     // Blocks run pad row by pad row (all sectors of row 0, then row 1, ...): blocks are dispatched in index order, so
     // the start list comes out roughly ordered by pad row.  K5 gives 32 consecutive start hits to a warp; tracklets
     // that start in the same row are in the same leg at the same time far more often than random ones, so the lanes

@@ -114,6 +114,19 @@ Layout make_layout(const tpc_tracker* t, int64_t maxClusters) {
     return L;
 }
 
+// Launch `kernel` on stream s, as the programmatic dependent of the kernel before it if pdl (the kernel then starts
+// when that one has triggered or finished, and waits for its completion itself: grid_dep_wait in device_types.cuh).
+template <class... KArgs, class... Args>
+cudaError_t launch_dep(bool pdl, void (*kernel)(KArgs...), int grid, int block, size_t smem, cudaStream_t s, Args... args) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)block); cfg.dynamicSmemBytes = smem; cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 void bind_pointers(tpc_tracker* t) {
     char* w = t->ws;
     const Layout& L = t->L;
@@ -491,26 +504,31 @@ int tpc_track_sectors(tpc_tracker* t) {
     CUDA_TRY(t, cudaEventRecord(t->ev[0], s));
     k1_sort_grid<<<NR, kK1Threads, sizeof(uint32_t) * (t->maxBinsLaunch + 1), s>>>(d);
     if (timed) CUDA_TRY(t, cudaEventRecord(t->ev[1], s));
-    k2_neighbours<<<NR, kK2Threads, 0, s>>>(d, dp);
+    // K2..K6: without events between them each kernel is launched as the programmatic dependent of the one before
+    // (its launch is set up while that one still runs; K5 also stages its row table meanwhile, device_types.cuh
+    // grid_dep_wait); with events they are ordinary launches.
+#ifndef TPC_PDL
+#define TPC_PDL 1
+#endif
+    const bool pdl = TPC_PDL && !timed;
+    const int k5Blocks = t->k5Blocks, phW = kK5PhasedThreads / 32;
+    CUDA_TRY(t, launch_dep(pdl, k2_neighbours, NR, kK2Threads, 0, s, d, dp));
     if (timed) CUDA_TRY(t, cudaEventRecord(t->ev[2], s));
-    k3_clean_start<<<NR, kK3Threads, 0, s>>>(d, dp);
+    CUDA_TRY(t, launch_dep(pdl, k3_clean_start, NR, kK3Threads, 0, s, d, dp));
     if (timed) CUDA_TRY(t, cudaEventRecord(t->ev[3], s));
-    {
-        // one persistent block per SM; the phased and the free-running instantiation decide on the device (from the
-        // number of start hits) which of them does the event, the other returns at once
-        const int blocks = t->k5Blocks;
-        if (t->k5SmemGrid) {
-            k5_construct_phased<true><<<blocks, kK5PhasedThreads, t->k5GridSmem, s>>>(d, dp);
-            k5_construct_free<true><<<blocks, kK5Threads, t->k5GridSmem, s>>>(d, dp, kK5PhasedThreads / 32);
-        } else {
-            k5_construct_phased<false><<<blocks, kK5PhasedThreads, 0, s>>>(d, dp);
-            k5_construct_free<false><<<blocks, kK5Threads, 0, s>>>(d, dp, kK5PhasedThreads / 32);
-        }
+    // K5: one persistent block per SM; the phased and the free-running instantiation decide on the device (from the
+    // number of start hits) which of them does the event, the other returns at once
+    if (t->k5SmemGrid) {
+        CUDA_TRY(t, launch_dep(pdl, k5_construct_phased<true>, k5Blocks, kK5PhasedThreads, t->k5GridSmem, s, d, dp));
+        CUDA_TRY(t, launch_dep(pdl, k5_construct_free<true>, k5Blocks, kK5Threads, t->k5GridSmem, s, d, dp, phW));
+    } else {
+        CUDA_TRY(t, launch_dep(pdl, k5_construct_phased<false>, k5Blocks, kK5PhasedThreads, 0, s, d, dp));
+        CUDA_TRY(t, launch_dep(pdl, k5_construct_free<false>, k5Blocks, kK5Threads, 0, s, d, dp, phW));
     }
     if (timed) CUDA_TRY(t, cudaEventRecord(t->ev[4], s));
-    k6_weights<<<t->k6aBlocks, kK6Threads, 0, s>>>(d, dp, t->k5Blocks);
+    CUDA_TRY(t, launch_dep(pdl, k6_weights, t->k6aBlocks, kK6Threads, 0, s, d, dp, k5Blocks));
     if (timed) CUDA_TRY(t, cudaEventRecord(t->ev[5], s));
-    k6_select<<<2 * t->k6Blocks, kK6Threads, 0, s>>>(d, dp);   // measured: 2 waves of warps beat 1 here (45 vs 50 us), not in K6a
+    CUDA_TRY(t, launch_dep(pdl, k6_select, 2 * t->k6Blocks, kK6Threads, 0, s, d, dp));   // measured: 2 waves of warps beat 1 here (45 vs 50 us), not in K6a
     CUDA_TRY(t, cudaEventRecord(t->ev[6], s));
     CUDA_TRY(t, cudaGetLastError());
     t->tracked = true; t->fetched = false;
