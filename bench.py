@@ -360,6 +360,9 @@ def main():
             ti.set_stream(sti.cuda_stream)
             ti.allocate_workspace(ev.n_clusters, device=dev)
         pipes.append((ti, torch.from_numpy(ev.y.copy()).pin_memory(), torch.from_numpy(ev.z.copy()).pin_memory()))
+    if n_pipe > 1:
+        for ti, _, _ in pipes:
+            ti.set_dependent_launch(False)     # several trackers on concurrent streams: ordinary launches (tpctrk.h)
     last = [None] * n_pipe
 
     def e2e_worker(i, n):
@@ -423,7 +426,7 @@ def main():
                    "kernel_times": "second pass of the same K steps with a CUDA event between the kernels (tpc_set_kernel_timing)"},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms_max, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "steps": n_e2e, "pipeline": "4 tracker instances / host threads / streams: copies of one event overlap the kernels of the others"},
+                "steps": n_e2e, "pipeline": f"{n_pipe} tracker instances / host threads / streams: copies of one event overlap the kernels of the others; ordinary (not dependent) launches"},
         "gpu_launches": args.steps * trk.launches_per_track(),
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": round(achieved, 2), "peak": peak, "unit": "GB/s",
                      "frac": round(achieved / peak, 5), "traffic": traffic, "peak_source": peak_src,

@@ -79,6 +79,7 @@ def lib():
         L.tpc_tracker_destroy.restype = None
         L.tpc_set_stream.argtypes = [vp, vp]
         L.tpc_set_kernel_timing.argtypes = [vp, ctypes.c_int]
+        L.tpc_set_dependent_launch.argtypes = [vp, ctypes.c_int]
         L.tpc_workspace_bytes.argtypes = [vp, i64]
         L.tpc_workspace_bytes.restype = ctypes.c_size_t
         L.tpc_set_workspace.argtypes = [vp, vp, ctypes.c_size_t]
@@ -162,6 +163,9 @@ class Tracker:
 
     def set_kernel_timing(self, on: bool):
         self._check(self._L.tpc_set_kernel_timing(self._h, 1 if on else 0), "tpc_set_kernel_timing")
+
+    def set_dependent_launch(self, on: bool):
+        self._check(self._L.tpc_set_dependent_launch(self._h, 1 if on else 0), "tpc_set_dependent_launch")
 
     def workspace_bytes(self, max_clusters: int) -> int:
         return int(self._L.tpc_workspace_bytes(self._h, int(max_clusters)))

@@ -35,6 +35,7 @@ struct tpc_tracker {
     float bz = 0.f, CB = 0.f;
     cudaStream_t stream = nullptr;
     int lastCuda = 0;
+    bool dependentLaunch = true;                     // tpc_set_dependent_launch
     bool kernelTiming = false, timedCall = false;   // tpc_set_kernel_timing; whether the last call recorded ev[1..5]
 
     // workspace
@@ -396,6 +397,12 @@ int tpc_set_kernel_timing(tpc_tracker* t, int on) {
     return TPC_OK;
 }
 
+int tpc_set_dependent_launch(tpc_tracker* t, int on) {
+    if (!t) return TPC_E_ARG;
+    t->dependentLaunch = on != 0;
+    return TPC_OK;
+}
+
 int tpc_set_stream(tpc_tracker* t, void* cuda_stream) {
     if (!t) return TPC_E_ARG;
     t->stream = (cudaStream_t)cuda_stream;
@@ -510,7 +517,7 @@ int tpc_track_sectors(tpc_tracker* t) {
 #ifndef TPC_PDL
 #define TPC_PDL 1
 #endif
-    const bool pdl = TPC_PDL && !timed;
+    const bool pdl = TPC_PDL && !timed && t->dependentLaunch;
     const int k5Blocks = t->k5Blocks, phW = kK5PhasedThreads / 32;
     CUDA_TRY(t, launch_dep(pdl, k2_neighbours, NR, kK2Threads, 0, s, d, dp));
     if (timed) CUDA_TRY(t, cudaEventRecord(t->ev[2], s));

@@ -347,8 +347,12 @@ def test_repeated_calls_give_identical_tracks():
     t0, l0 = _canonical_tracks(tracks.copy(), ids.copy())
     st0 = trk.get_stats()
     assert st0["k6a_fused"]
-    for _ in range(4):
+    for rep in range(4):
+        # the launch options change how the kernels are launched, never what they compute (tpctrk.h)
+        trk.set_kernel_timing(rep == 1)
+        trk.set_dependent_launch(rep != 2)
         _, t, i = run_gpu(ev, tracker=trk)
+        assert (trk.get_stats()["kernel_us"]["K5_construct"] > 0) == (rep == 1)
         t1, l1 = _canonical_tracks(t, i)
         st = trk.get_stats()
         for k in ("n_links", "n_start_hits", "n_tracklets", "n_tracklet_hits", "n_tracks", "n_track_clusters"):
