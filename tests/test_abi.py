@@ -70,8 +70,14 @@ def test_calls_out_of_order_fail_without_touching_the_gpu():
     with pytest.raises(binding.TpcError) as e:
         t.load_clusters(5, 0, None, y, y)
     assert e.value.code == binding.TPC_E_ARG
+    # the launch options are host state only: settable before any workspace exists, NULL handle is an argument error
+    t.set_kernel_timing(True); t.set_kernel_timing(False)
+    t.set_dependent_launch(False); t.set_dependent_launch(True)
+    assert binding.lib().tpc_set_kernel_timing(None, 1) == binding.TPC_E_ARG
+    assert binding.lib().tpc_set_dependent_launch(None, 1) == binding.TPC_E_ARG
     st = t.get_stats()
     assert st["n_clusters"] == 0 and st["n_tracks"] == 0
+    assert st["k6a_fused"] is False
     assert binding.lib().tpc_strerror(binding.TPC_E_OVERFLOW).decode() == "tracklet capacity exceeded"
 
 
