@@ -21,7 +21,7 @@ __device__ __forceinline__ int bin_of(float v, float v0, float inv, int n) {
 #define TPC_ZF 2.4f   /* measured on config 3 (K5 us): 1.5 -> 847, 1.8 -> 590, 2.2 -> 497, 2.6 -> 509; the steep side is the low one */
 #endif
 #ifndef TPC_K1T
-#define TPC_K1T 256
+#define TPC_K1T 192
 #endif
 constexpr int kK1Threads = TPC_K1T;
 constexpr int kK1Stage = 512;     // 8 KB of static shared memory beside the <= 32 KB dynamic histogram (48 KB limit)
