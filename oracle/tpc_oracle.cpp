@@ -16,7 +16,13 @@
  * Pins (tests/test_oracle_*.py): brute force == grid; analytic circle, group property and
  * finite-difference Jacobian of the propagation; closed-form least squares for the filter;
  * noise-free straight/helix recovery; pulls and chi2/ndf; chain/selector invariants; clean
- * single-track events found with all clusters.  No function here is "parity unpinned".
+ * single-track events found with all clusters; and for the control logic of constructTracklets /
+ * roadSearch / selectTracklets (tests/test_oracle_legs.py): hand-counted gap bridging in legs B
+ * and D (4 empty rows crossed, the 5th stops; counter from 0 at r0; leg C neither searches nor
+ * counts), 9-vs-10 hits for kept tracklets and for owned hits, the road edge at
+ * nsig*sqrt(C+err2) from the closed-form variance of a line fit, its cap and its rectangular
+ * shape, the load-index tie-break of the search, and the restart of the inward pass against an
+ * independent numpy filter.  No function here is "parity unpinned".
  *
  * Templated on the scalar type: double for the 1e-5 self-checks, float for GPU parity
  * (build with -O2 -ffp-contract=off: IEEE fp32; a fused multiply-add happens exactly where std::fma is written,
