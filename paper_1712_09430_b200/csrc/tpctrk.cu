@@ -12,7 +12,6 @@
 #include "device_types.cuh"
 #include "kernels_ca.cuh"
 #include "kernels_kf.cuh"
-#include "kernels_k5pool.cuh"
 
 using namespace tpc;
 
@@ -23,7 +22,7 @@ inline size_t align_up(size_t v, size_t a = kAlign) { return (v + a - 1) / a * a
 
 struct Layout {   // byte offsets into the workspace
     size_t inY, inZ, grid, meta, rowX, hits, orig, binStart, buckets, linkUp, linkDn, linkUpC, linkDnC, weight, starts, startsRaw, rowHist, rowStartBase, recs, rowHit,
-        live, tracks, clusterIds, counters, sectorGidBase, total;
+        tracks, clusterIds, counters, sectorGidBase, total;
     int64_t hitCap, binCap, maxTracklets;
 };
 
@@ -69,8 +68,6 @@ struct tpc_tracker {
     bool haveEvents = false;
     float kernelUs[8] = {0};
     int k5Blocks = 0, k6Blocks = 0, k6aBlocks = 0;
-    int k5Mode = 0;                                  // 1 (TPC_K5_MODE=1): pooled kernel (kernels_k5pool.cuh), an experiment
-    TrackletLive* live = nullptr;
     size_t k5GridSmem = 0; bool k5SmemGrid = false;
 };
 
@@ -110,7 +107,6 @@ Layout make_layout(const tpc_tracker* t, int64_t maxClusters) {
     L.rowStartBase = take(sizeof(uint32_t) * (kMaxRows + 2));
     L.recs = take(sizeof(TrackletRec) * L.maxTracklets);
     L.rowHit = take(sizeof(int32_t) * L.maxTracklets * t->rhStride);
-    L.live = take(sizeof(TrackletLive) * L.maxTracklets);
     L.tracks = take(sizeof(tpc_track) * L.maxTracklets);
     L.clusterIds = take(sizeof(uint32_t) * (maxClusters + 16));
     L.counters = take(sizeof(uint32_t) * (kNCounters + kMaxPending));
@@ -143,7 +139,6 @@ void bind_pointers(tpc_tracker* t) {
     d.linkUpC = (int32_t*)(w + L.linkUpC); d.linkDnC = (int32_t*)(w + L.linkDnC);
     d.weight = (uint32_t*)(w + L.weight); d.starts = (int4*)(w + L.starts); d.startsRaw = (int4*)(w + L.startsRaw); d.rowHist = (uint32_t*)(w + L.rowHist); d.rowStartBase = (const uint32_t*)(w + L.rowStartBase);
     d.recs = (TrackletRec*)(w + L.recs); d.rowHit = (int32_t*)(w + L.rowHit);
-    t->live = (TrackletLive*)(w + L.live);
     d.tracks = (tpc_track*)(w + L.tracks); d.clusterIds = (uint32_t*)(w + L.clusterIds);
     d.counters = (uint32_t*)(w + L.counters); d.sectorGidBase = (uint32_t*)(w + L.sectorGidBase);
     d.nRowsTotal = t->nRowsTotal; d.maxTracklets = (int32_t)std::min<int64_t>(L.maxTracklets, 0x7fffffff);
@@ -372,7 +367,6 @@ int tpc_tracker_create(const tpc_geometry* g, float bz_tesla, tpc_tracker** out)
         !(t->P.grid_bins_per_hit >= 0.25f && t->P.grid_bins_per_hit <= 64.f)) {
         delete t; return TPC_E_ARG;
     }
-    if (const char* m = getenv("TPC_K5_MODE")) t->k5Mode = atoi(m);
     t->bz = bz_tesla;
     t->CB = (float)(-0.299792458e-2 * (double)bz_tesla);   // kappa = (q/pT) * CB, constant field
     t->rowN.assign(t->nRowsTotal, 0); t->rowIn.assign(t->nRowsTotal, 0);
@@ -448,7 +442,6 @@ int tpc_set_workspace(tpc_tracker* t, void* dev_ptr, size_t bytes) {
         if (t->k5SmemGrid) {
             CUDA_TRY(t, cudaFuncSetAttribute(k5_construct_free<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->k5GridSmem));
             CUDA_TRY(t, cudaFuncSetAttribute(k5_construct_phased<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->k5GridSmem));
-            CUDA_TRY(t, cudaFuncSetAttribute(k5_construct_pool<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->k5GridSmem));
         }
         occ5 = 1;   // one persistent block per SM (both instantiations must see the same grid)
         CUDA_TRY(t, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ6, k6_select, kK6Threads, 0));
@@ -532,22 +525,16 @@ int tpc_track_sectors(tpc_tracker* t) {
     if (timed) CUDA_TRY(t, cudaEventRecord(t->ev[3], s));
     // K5: one persistent block per SM; the phased and the free-running instantiation decide on the device (from the
     // number of start hits) which of them does the event, the other returns at once
-    if (t->k5Mode == 1) {
-        if (t->k5SmemGrid) CUDA_TRY(t, launch_dep(pdl, k5_construct_pool<true>, k5Blocks, kK5PoolThreads, t->k5GridSmem, s, d, dp, t->live));
-        else CUDA_TRY(t, launch_dep(pdl, k5_construct_pool<false>, k5Blocks, kK5PoolThreads, 0, s, d, dp, t->live));
-        if (timed) { CUDA_TRY(t, cudaEventRecord(t->ev[4], s)); CUDA_TRY(t, cudaEventRecord(t->ev[5], s)); }
+    if (t->k5SmemGrid) {
+        CUDA_TRY(t, launch_dep(pdl, k5_construct_phased<true>, k5Blocks, kK5PhasedThreads, t->k5GridSmem, s, d, dp));
+        CUDA_TRY(t, launch_dep(pdl, k5_construct_free<true>, k5Blocks, kK5Threads, t->k5GridSmem, s, d, dp, phW));
     } else {
-        if (t->k5SmemGrid) {
-            CUDA_TRY(t, launch_dep(pdl, k5_construct_phased<true>, k5Blocks, kK5PhasedThreads, t->k5GridSmem, s, d, dp));
-            CUDA_TRY(t, launch_dep(pdl, k5_construct_free<true>, k5Blocks, kK5Threads, t->k5GridSmem, s, d, dp, phW));
-        } else {
-            CUDA_TRY(t, launch_dep(pdl, k5_construct_phased<false>, k5Blocks, kK5PhasedThreads, 0, s, d, dp));
-            CUDA_TRY(t, launch_dep(pdl, k5_construct_free<false>, k5Blocks, kK5Threads, 0, s, d, dp, phW));
-        }
-        if (timed) CUDA_TRY(t, cudaEventRecord(t->ev[4], s));
-        CUDA_TRY(t, launch_dep(pdl, k6_weights, t->k6aBlocks, kK6Threads, 0, s, d, dp, k5Blocks));
-        if (timed) CUDA_TRY(t, cudaEventRecord(t->ev[5], s));
+        CUDA_TRY(t, launch_dep(pdl, k5_construct_phased<false>, k5Blocks, kK5PhasedThreads, 0, s, d, dp));
+        CUDA_TRY(t, launch_dep(pdl, k5_construct_free<false>, k5Blocks, kK5Threads, 0, s, d, dp, phW));
     }
+    if (timed) CUDA_TRY(t, cudaEventRecord(t->ev[4], s));
+    CUDA_TRY(t, launch_dep(pdl, k6_weights, t->k6aBlocks, kK6Threads, 0, s, d, dp, k5Blocks));
+    if (timed) CUDA_TRY(t, cudaEventRecord(t->ev[5], s));
     CUDA_TRY(t, launch_dep(pdl, k6_select, 2 * t->k6Blocks, kK6Threads, 0, s, d, dp));   // measured: 2 waves of warps beat 1 here (45 vs 50 us), not in K6a
     CUDA_TRY(t, cudaEventRecord(t->ev[6], s));
     CUDA_TRY(t, cudaGetLastError());
@@ -574,7 +561,7 @@ int tpc_sync(tpc_tracker* t) {
     // [7]: 1 if this event was the phased K5 kernel's, whose warps run the K6a weights pass themselves (same test as
     // k5_phased_mode on the device); K6a's own launch then only did the few groups the last warps left to it
     const unsigned nTotal = (unsigned)std::min<int64_t>(t->counters[kNStart], t->dev.maxTracklets);
-    t->kernelUs[7] = t->k5Mode == 1 ? 1.f : (TPC_K5_FUSE_K6A && (float)nTotal / (32.0f * (float)t->k5Blocks) <= (float)(kK5PhasedThreads / 32)) ? 1.f : 0.f;
+    t->kernelUs[7] = (TPC_K5_FUSE_K6A && (float)nTotal / (32.0f * (float)t->k5Blocks) <= (float)(kK5PhasedThreads / 32)) ? 1.f : 0.f;
     return TPC_OK;
 }
 
