@@ -110,7 +110,10 @@ enum {
 void tpc_default_params(tpc_params* p);
 
 /* Create a tracker for a geometry and a constant field Bz [T].  g and its pointers are host
- * memory, copied.  *out is owned by the library until tpc_tracker_destroy.  Does not touch the GPU. */
+ * memory, copied.  *out is owned by the library until tpc_tracker_destroy.  Does not touch the GPU.
+ * TPC_E_ARG for an unsupported geometry and for parameters outside their domain: variances (err2_*, kf_c**0),
+ * road_nsig, road_max and max_tracklets_per_cluster must be positive and finite, kf_smax inside (0,1), the nf_* window
+ * constants non-negative, min_hits >= 1, max_gap >= 0, seed_min_chain >= 2, grid_bins_per_hit in [0.25, 64]. */
 int tpc_tracker_create(const tpc_geometry* g, float bz_tesla, tpc_tracker** out);
 void tpc_tracker_destroy(tpc_tracker* t);
 
@@ -142,8 +145,11 @@ int tpc_reset_event(tpc_tracker* t);
  * (device: enqueued on the stream; host: staged in pinned memory, uploaded by tpc_track_sectors).  x may be NULL and
  * is not used: the tracker takes the pad-row x (R-13).  Index i in this call is the cluster's load index;
  * its event-global id is rowBase(sector,row)+i with rowBase the exclusive prefix sum of the loaded counts in
- * ascending (sector,row) order.  Loading a (sector,row) again replaces it.  Non-finite coordinates give undefined
- * tracks but never a crash or hang. */
+ * ascending (sector,row) order.  Loading a (sector,row) again replaces it: in place if the new load is not larger than
+ * the largest earlier load of that (sector,row) since the last reset, otherwise appended - the old staging slots then
+ * count against max_clusters until tpc_reset_event.
+ * Returns TPC_E_NOMEM when the staging area is full.  Non-finite coordinates give undefined tracks but never a crash
+ * or hang. */
 int tpc_load_clusters(tpc_tracker* t, int sector, int row, int n, const float* x, const float* y, const float* z);
 
 /* Load a whole event at once: row_counts[n_sectors*n_rows] on the host; y, z concatenated in ascending (sector,row)

@@ -3,6 +3,7 @@
 // the workspace, stages input, launches K1..K6 on the caller's stream and downloads the compacted result.
 // There is no CPU fallback: without a device the compute calls return TPC_E_CUDA.
 #include <algorithm>
+#include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -46,7 +47,7 @@ struct tpc_tracker {
     DevPtrs dev{};
 
     // loaded event (host bookkeeping)
-    std::vector<int32_t> rowN, rowIn;       // per (sector,row): count, staging offset
+    std::vector<int32_t> rowN, rowIn, rowCap;   // per (sector,row): count, staging offset, slots reserved at that offset
     int64_t cursor = 0;                     // next free staging slot
     int64_t nClusters = 0;
     bool finalized = false, tracked = false, fetched = false;
@@ -250,6 +251,10 @@ int finalize_event(tpc_tracker* t) {
 int stage_clusters(tpc_tracker* t, int64_t at, int64_t n, const float* y, const float* z) {
     if (n == 0) return TPC_OK;
     if (is_device_pointer(y)) {
+        if (t->dirtyHi > t->dirtyLo && at < t->dirtyHi && at + n > t->dirtyLo) {   // a row replaced in place: the pending
+            int rc = flush_dirty(t);                                              // host range must not overwrite it later
+            if (rc != TPC_OK) return rc;
+        }
         CUDA_TRY(t, cudaMemcpyAsync((float*)t->dev.inY + at, y, sizeof(float) * n, cudaMemcpyDeviceToDevice, t->stream));
         CUDA_TRY(t, cudaMemcpyAsync((float*)t->dev.inZ + at, z, sizeof(float) * n, cudaMemcpyDeviceToDevice, t->stream));
     } else if (n >= (1 << 16) && is_pinned_host_pointer(y) && is_pinned_host_pointer(z)) {
@@ -363,13 +368,22 @@ int tpc_tracker_create(const tpc_geometry* g, float bz_tesla, tpc_tracker** out)
     t->rhStride = (g->n_rows + 31) / 32 * 32;
     t->rowX.assign(g->row_x, g->row_x + g->n_rows);
     if (g->params) t->P = *g->params; else tpc_default_params(&t->P);
-    if (t->P.seed_min_chain < 2 || t->P.min_hits < 1 || t->P.max_gap < 0 || !(t->P.max_tracklets_per_cluster > 0.f) ||
-        !(t->P.grid_bins_per_hit >= 0.25f && t->P.grid_bins_per_hit <= 64.f)) {
-        delete t; return TPC_E_ARG;
+    {
+        // the kernels' branch-free reciprocals and square roots assume positive finite variances and roads
+        // (kernels_kf.cuh rcp_rn_inrange / sqrt_rn_inrange): everything else is refused here
+        const tpc_params& P = t->P;
+        auto pos = [](float v) { return v > 0.f && v < 1e30f; };              // false for NaN, inf, <= 0
+        auto nonneg = [](float v) { return v >= 0.f && v < 1e30f; };
+        const bool ok = pos(P.err2_y) && pos(P.err2_z) && pos(P.kf_css0) && pos(P.kf_ctt0) && pos(P.kf_ckk0) &&
+                        pos(P.road_nsig) && pos(P.road_max) && P.kf_smax > 0.f && P.kf_smax < 1.f &&
+                        nonneg(P.nf_ty) && nonneg(P.nf_tz) && nonneg(P.nf_c) && nonneg(P.nf_d2max) &&
+                        P.seed_min_chain >= 2 && P.min_hits >= 1 && P.max_gap >= 0 && pos(P.max_tracklets_per_cluster) &&
+                        P.grid_bins_per_hit >= 0.25f && P.grid_bins_per_hit <= 64.f && bz_tesla == bz_tesla && std::abs(bz_tesla) < 1e3f;
+        if (!ok) { delete t; return TPC_E_ARG; }
     }
     t->bz = bz_tesla;
     t->CB = (float)(-0.299792458e-2 * (double)bz_tesla);   // kappa = (q/pT) * CB, constant field
-    t->rowN.assign(t->nRowsTotal, 0); t->rowIn.assign(t->nRowsTotal, 0);
+    t->rowN.assign(t->nRowsTotal, 0); t->rowIn.assign(t->nRowsTotal, 0); t->rowCap.assign(t->nRowsTotal, 0);
     *out = t;
     return TPC_OK;
 }
@@ -438,10 +452,21 @@ int tpc_set_workspace(tpc_tracker* t, void* dev_ptr, size_t bytes) {
         CUDA_TRY(t, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
         // K5 keeps the whole row table in shared memory when it fits (one block per SM)
         t->k5GridSmem = sizeof(RowGrid) * (size_t)t->nRowsTotal;
-        t->k5SmemGrid = t->k5GridSmem + 2048 <= 227 * 1024;
-        if (t->k5SmemGrid) {
-            CUDA_TRY(t, cudaFuncSetAttribute(k5_construct_free<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->k5GridSmem));
-            CUDA_TRY(t, cudaFuncSetAttribute(k5_construct_phased<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->k5GridSmem));
+        {
+            // dynamic + static shared memory of BOTH instantiations must fit the opt-in limit; otherwise (or if the
+            // attribute cannot be set) the same kernels read the table from global memory
+            int optin = 0;
+            CUDA_TRY(t, cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+            cudaFuncAttributes fa{}, fb{};
+            CUDA_TRY(t, cudaFuncGetAttributes(&fa, k5_construct_free<true>));
+            CUDA_TRY(t, cudaFuncGetAttributes(&fb, k5_construct_phased<true>));
+            const size_t stat = std::max(fa.sharedSizeBytes, fb.sharedSizeBytes);
+            t->k5SmemGrid = t->k5GridSmem + stat <= (size_t)optin;
+            if (t->k5SmemGrid) {
+                cudaError_t e1 = cudaFuncSetAttribute(k5_construct_free<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->k5GridSmem);
+                cudaError_t e2 = cudaFuncSetAttribute(k5_construct_phased<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->k5GridSmem);
+                if (e1 != cudaSuccess || e2 != cudaSuccess) { cudaGetLastError(); t->k5SmemGrid = false; }
+            }
         }
         occ5 = 1;   // one persistent block per SM (both instantiations must see the same grid)
         CUDA_TRY(t, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ6, k6_select, kK6Threads, 0));
@@ -458,6 +483,7 @@ int tpc_reset_event(tpc_tracker* t) {
     if (!t) return TPC_E_ARG;
     std::fill(t->rowN.begin(), t->rowN.end(), 0);
     std::fill(t->rowIn.begin(), t->rowIn.end(), 0);
+    std::fill(t->rowCap.begin(), t->rowCap.end(), 0);
     t->cursor = 0; t->nClusters = 0; t->dirtyLo = t->dirtyHi = 0;
     t->finalized = t->tracked = t->fetched = false;
     return TPC_OK;
@@ -468,12 +494,16 @@ int tpc_load_clusters(tpc_tracker* t, int sector, int row, int n, const float* x
     if (!t || sector < 0 || sector >= t->nSec || row < 0 || row >= t->nRows || n < 0) return TPC_E_ARG;
     if (n > 0 && (!y || !z)) return TPC_E_ARG;
     if (!t->ws) return TPC_E_STATE;
-    if (t->cursor + n > t->maxClusters) return TPC_E_NOMEM;
     const int i = sector * t->nRows + row;
-    int rc = stage_clusters(t, t->cursor, n, y, z);
+    // a (sector,row) that is loaded again keeps its staging slots if the new load fits the slots reserved for it, else
+    // it is appended (the old slots stay unused until tpc_reset_event; tpctrk.h)
+    const bool reuse = n <= t->rowCap[i];
+    if (!reuse && t->cursor + n > t->maxClusters) return TPC_E_NOMEM;
+    const int64_t at = reuse ? t->rowIn[i] : t->cursor;
+    int rc = stage_clusters(t, at, n, y, z);
     if (rc != TPC_OK) return rc;
-    t->rowN[i] = n; t->rowIn[i] = (int32_t)t->cursor;
-    t->cursor += n;
+    t->rowN[i] = n; t->rowIn[i] = (int32_t)at;
+    if (!reuse) { t->rowCap[i] = n; t->cursor += n; }
     t->finalized = t->tracked = t->fetched = false;
     return TPC_OK;
 }
@@ -490,7 +520,7 @@ int tpc_load_event(tpc_tracker* t, const int32_t* row_counts, const float* y, co
     if (total > t->maxClusters) return TPC_E_NOMEM;
     tpc_reset_event(t);
     int64_t off = 0;
-    for (int i = 0; i < t->nRowsTotal; i++) { t->rowN[i] = row_counts[i]; t->rowIn[i] = (int32_t)off; off += row_counts[i]; }
+    for (int i = 0; i < t->nRowsTotal; i++) { t->rowN[i] = t->rowCap[i] = row_counts[i]; t->rowIn[i] = (int32_t)off; off += row_counts[i]; }
     t->cursor = total;
     int rc = stage_clusters(t, 0, total, y, z);
     if (rc != TPC_OK) return rc;

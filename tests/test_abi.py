@@ -54,6 +54,29 @@ def test_create_validates_geometry():
         binding.Tracker(36, 159, rx, 0.5, p)
 
 
+def test_parameters_outside_their_domain_are_refused():
+    """The kernels' branch-free reciprocal / square root assume positive finite variances and roads:
+    anything else must be TPC_E_ARG at create, never silent garbage."""
+    rx = np.linspace(85, 246, 159).astype(np.float32)
+    bad = [("err2_y", 0.0), ("err2_z", -0.01), ("err2_y", float("nan")), ("kf_css0", 0.0), ("kf_ctt0", float("inf")),
+           ("kf_ckk0", -1.0), ("road_nsig", 0.0), ("road_max", -2.0), ("road_max", float("nan")), ("kf_smax", 0.0),
+           ("kf_smax", 1.0), ("kf_smax", 1.5), ("kf_smax", float("nan")), ("nf_ty", -1.0), ("nf_tz", float("nan")),
+           ("nf_c", -0.5), ("nf_d2max", -1.0), ("min_hits", 0), ("max_gap", -1), ("max_tracklets_per_cluster", 0.0),
+           ("grid_bins_per_hit", 0.1), ("grid_bins_per_hit", 100.0)]
+    for name, val in bad:
+        p = binding.default_params()
+        setattr(p, name, val)
+        with pytest.raises(binding.TpcError) as e:
+            binding.Tracker(36, 159, rx, 0.5, p)
+        assert e.value.code == binding.TPC_E_ARG, (name, val)
+    with pytest.raises(binding.TpcError):
+        binding.Tracker(36, 159, rx, float("nan"))
+    # the defaults and a few legal corner values pass
+    p = binding.default_params()
+    p.nf_c, p.max_gap, p.kf_smax = 0.0, 0, 0.999
+    binding.Tracker(36, 159, rx, 0.0, p).destroy()
+
+
 def test_calls_out_of_order_fail_without_touching_the_gpu():
     rx = np.linspace(85, 246, 159).astype(np.float32)
     t = binding.Tracker(2, 159, rx, 0.5)

@@ -536,3 +536,59 @@ def test_time_per_cluster_is_about_linear(capsys):
         assert table[4][k] <= 1.5 * table[3][k], (k, table[3][k], table[4][k])
     # (K6a runs inside K5 for one event and as its own launch for the time frame: only K6b is comparable)
     assert table[4]["K6b_ns_per_tracklet_hit"] <= 1.5 * table[3]["K6b_ns_per_tracklet_hit"]
+
+
+def test_row_table_just_beyond_the_shared_memory_limit_falls_back():
+    """45 x 160 = 7200 (sector,row) entries need 230,400 bytes of dynamic shared memory - below 227 KB + 2 KB
+    of slack but, with the kernels' ~3 KB of static shared memory, above the 232,448-byte opt-in limit.  The library
+    must run the global-table instantiation instead of failing in tpc_set_workspace."""
+    _cuda()
+    n_sec, n_rows = 45, 160
+    rx = (85.0 + 1.0 * np.arange(n_rows)).astype(np.float32)
+    rng = np.random.default_rng(12)
+    hits = []
+    for _ in range(120):
+        s = int(rng.integers(0, n_sec))
+        a, b = rng.uniform(-8, 8), rng.uniform(-0.1, 0.1)
+        c, dz = rng.uniform(5, 120), rng.uniform(-0.4, 0.4)
+        for r in range(int(rng.integers(0, 60)), n_rows):
+            x = float(rx[r])
+            hits.append((s, r, a + b * (x - 85.0) + rng.normal(0, 0.1), c + dz * (x - 85.0) + rng.normal(0, 0.1)))
+    for _ in range(3000):
+        hits.append((int(rng.integers(0, n_sec)), int(rng.integers(0, n_rows)), rng.uniform(-15, 15), rng.uniform(0, 250)))
+    ev = datagen.event_from_hits(hits, n_sec, rx)
+    ref = oracle.run_event(ev)
+    assert ref.tracks.size > 50
+    trk, tracks, ids = run_gpu(ev)
+    out = compare(ev, trk, tracks, ids, ref)
+    assert out["tracklet_mismatch"] == 0 and out["link_mismatch_0"] == 0
+
+
+def test_reloading_rows_in_place_does_not_use_up_the_staging_area():
+    """tpctrk.h: a (sector,row) loaded again keeps its slots when the new load is not larger.  Every row of the event
+    (largest so far) is loaded 30 times, with varying lengths, into a workspace sized for ONE event: it would overflow
+    30-fold if reloads were appended."""
+    torch = _cuda()
+    ev = datagen.config_event(1, seed=8)
+    ref = oracle.run_event(ev)
+    trk = binding.Tracker(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz)
+    trk.set_stream(torch.cuda.current_stream().cuda_stream)
+    trk.allocate_workspace(ev.n_clusters)
+    base = ev.row_base
+    rng = np.random.default_rng(3)
+    for rep in range(30):
+        last = rep == 29
+        for sr in range(ev.n_sectors * ev.n_rows):
+            lo, hi = int(base[sr]), int(base[sr + 1])
+            if hi == lo:
+                continue
+            s, r = divmod(sr, ev.n_rows)
+            if last or rep == 0:                         # (the first load reserves the row's slots)
+                trk.load_clusters(s, r, None, ev.y[lo:hi], ev.z[lo:hi])
+            else:                                        # junk, now and then shorter
+                k = max(1, hi - lo - (rep % 3))
+                junk = rng.uniform(-5, 5, k).astype(np.float32)
+                trk.load_clusters(s, r, None, junk, junk)
+    trk.track_sectors()
+    tracks, ids = trk.get_tracks()
+    compare(ev, trk, tracks, ids, ref)
