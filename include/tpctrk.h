@@ -85,6 +85,8 @@ typedef struct tpc_track {
 typedef struct tpc_stats {
     int64_t n_clusters, n_links, n_start_hits, n_tracklets, n_tracklet_hits, n_tracks, n_track_clusters;
     int64_t workspace_bytes_used, max_clusters, max_tracklets;
+    int64_t n_output_refetches; /* calls of tpc_get_tracks (since create) that had to fetch a remainder because the
+                                 download queued by tpc_track_sectors was estimated too small */
     float kernel_us[8];       /* K1 sort+grid, K2 neighbours, K3/K4 clean+start, K5 construct, K6a weights,
                                  K6b select+compact, [6] = K1..K6 total, [7] = 1.0 if the K6a weights pass of this
                                  event ran inside the K5 launch (about one tracklet per GPU thread or fewer: [3]
@@ -153,20 +155,35 @@ int tpc_reset_event(tpc_tracker* t);
 int tpc_load_clusters(tpc_tracker* t, int sector, int row, int n, const float* x, const float* y, const float* z);
 
 /* Load a whole event at once: row_counts[n_sectors*n_rows] on the host; y, z concatenated in ascending (sector,row)
- * order, both host or both device pointers.  Replaces everything loaded before. */
+ * order, both host or both device pointers.  Replaces everything loaded before.
+ * Ownership of y, z: ordinary host memory and device memory are copied (or the copy is ordered on the stream) before
+ * the call returns.  PAGE-LOCKED host memory of 64 Ki clusters or more is read by DMA directly and the call returns
+ * as soon as that copy is QUEUED (DMA runs beside the kernels): the buffers must stay untouched until
+ * tpc_wait_input, tpc_sync or tpc_get_tracks has returned.  The same holds for tpc_load_clusters. */
 int tpc_load_event(tpc_tracker* t, const int32_t* row_counts, const float* y, const float* z);
 
-/* Run K1..K6 (sort+grid, neighbours finder, cleaner+start hits, tracklet constructor, selector+compaction) on the
- * stream.  Asynchronous.  May be called repeatedly on the same loaded event. */
-int tpc_track_sectors(tpc_tracker* t);
+/* Block until every input buffer handed to tpc_load_clusters / tpc_load_event so far has been read. */
+int tpc_wait_input(tpc_tracker* t);
 
-/* Synchronise, download the result into library-owned pinned memory (valid until the next track/reset/destroy).
+/* Run K1..K6 (sort+grid, neighbours finder, cleaner+start hits, tracklet constructor, selector+compaction) on the
+ * stream.  Asynchronous.  May be called repeatedly on the same loaded event.
+ * Output of unknown size ("the tracker can estimate a buffer that is large enough to store all tracks
+ * and queue the transfer of this buffer immediately ... if the estimation was too small, the tracker can still
+ * fetch the rest"): behind K6 the call queues the download of the counters and of an estimated prefix of the tracks
+ * and cluster ids (first event: one track per 64 clusters and one id per cluster; afterwards the last fetched
+ * event's counts + 25 %) into library-owned pinned memory.  tpc_set_output_prefetch(t, 0) queues the counters only. */
+int tpc_track_sectors(tpc_tracker* t);
+int tpc_set_output_prefetch(tpc_tracker* t, int on);
+
+/* Wait (once, on an event behind the queued download; the stream may hold later work) and hand out the result in
+ * library-owned pinned memory (valid until the next track/reset/destroy).  Copies only the remainder, if the queued
+ * estimate was short (tpc_stats.n_output_refetches counts those calls).
  * tracks[i].cluster_offset indexes cluster_ids (event-global ids).  Track order is unspecified.
  * Returns TPC_E_OVERFLOW if the tracklet capacity was exceeded (results then cover the first max_tracklets seeds). */
 int tpc_get_tracks(tpc_tracker* t, const tpc_track** tracks, int32_t* n_tracks,
                    const uint32_t** cluster_ids, int64_t* n_cluster_ids);
 
-/* Synchronise the stream and fetch counters + per-kernel device times only (no track download). */
+/* Wait for the last tpc_track_sectors and its queued download; counters + per-kernel device times only. */
 int tpc_sync(tpc_tracker* t);
 int tpc_get_stats(tpc_tracker* t, tpc_stats* out);
 

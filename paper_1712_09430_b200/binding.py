@@ -38,7 +38,8 @@ class tpc_stats(ctypes.Structure):
         ("n_clusters", ctypes.c_int64), ("n_links", ctypes.c_int64), ("n_start_hits", ctypes.c_int64),
         ("n_tracklets", ctypes.c_int64), ("n_tracklet_hits", ctypes.c_int64), ("n_tracks", ctypes.c_int64),
         ("n_track_clusters", ctypes.c_int64), ("workspace_bytes_used", ctypes.c_int64),
-        ("max_clusters", ctypes.c_int64), ("max_tracklets", ctypes.c_int64), ("kernel_us", ctypes.c_float * 8),
+        ("max_clusters", ctypes.c_int64), ("max_tracklets", ctypes.c_int64), ("n_output_refetches", ctypes.c_int64),
+        ("kernel_us", ctypes.c_float * 8),
     ]
 
 
@@ -80,6 +81,8 @@ def lib():
         L.tpc_set_stream.argtypes = [vp, vp]
         L.tpc_set_kernel_timing.argtypes = [vp, ctypes.c_int]
         L.tpc_set_dependent_launch.argtypes = [vp, ctypes.c_int]
+        L.tpc_set_output_prefetch.argtypes = [vp, ctypes.c_int]
+        L.tpc_wait_input.argtypes = [vp]
         L.tpc_workspace_bytes.argtypes = [vp, i64]
         L.tpc_workspace_bytes.restype = ctypes.c_size_t
         L.tpc_set_workspace.argtypes = [vp, vp, ctypes.c_size_t]
@@ -166,6 +169,12 @@ class Tracker:
 
     def set_dependent_launch(self, on: bool):
         self._check(self._L.tpc_set_dependent_launch(self._h, 1 if on else 0), "tpc_set_dependent_launch")
+
+    def set_output_prefetch(self, on: bool):
+        self._check(self._L.tpc_set_output_prefetch(self._h, 1 if on else 0), "tpc_set_output_prefetch")
+
+    def wait_input(self):
+        return self._check(self._L.tpc_wait_input(self._h), "tpc_wait_input")
 
     def workspace_bytes(self, max_clusters: int) -> int:
         return int(self._L.tpc_workspace_bytes(self._h, int(max_clusters)))

@@ -54,6 +54,12 @@ struct tpc_tracker {
     float* hostY = nullptr; float* hostZ = nullptr; int64_t hostCap = 0;   // pinned mirror for host-pointer loads
     int64_t dirtyLo = 0, dirtyHi = 0;       // host-staged range not yet uploaded
     cudaEvent_t evUpload = nullptr; bool uploadPending = false;
+    cudaEvent_t evTables = nullptr; bool tablesPending = false;   // upload of the host row tables of the last finalize
+    cudaEvent_t evDone = nullptr;           // after the result download queued behind K6 (tpc_track_sectors)
+    int64_t estTracks = 0, estIds = 0;      // size of the download that is queued before the counts are known
+    int64_t queuedTracks = 0, queuedIds = 0;   // ... what the last tpc_track_sectors queued
+    bool queueOutput = true;                // tpc_set_output_prefetch
+    int64_t nRefetch = 0;                   // how often the estimate was short (tpc_stats)
     RowGrid* hostGrid = nullptr;            // pinned
     RowMeta* hostMeta = nullptr;            // pinned
     uint32_t* hostSectorBase = nullptr;     // pinned
@@ -202,8 +208,10 @@ int finalize_event(tpc_tracker* t) {
         CUDA_TRY(t, cudaMallocHost(&t->hostSectorBase, sizeof(uint32_t) * (t->nSec + 1)));
         CUDA_TRY(t, cudaMallocHost(&t->hostCounters, sizeof(uint32_t) * kNCounters));
         CUDA_TRY(t, cudaMallocHost(&t->hostRowStartBase, sizeof(uint32_t) * (kMaxRows + 2)));
-    } else {
-        CUDA_TRY(t, cudaStreamSynchronize(t->stream));   // a previous async upload may still read the host tables
+        CUDA_TRY(t, cudaEventCreateWithFlags(&t->evTables, cudaEventDisableTiming));
+    } else if (t->tablesPending) {
+        CUDA_TRY(t, cudaEventSynchronize(t->evTables));  // the previous upload may still read the host tables (the
+        t->tablesPending = false;                        // kernels behind it are not waited for)
     }
     int64_t gid = 0, hitOff = 0, binOff = 0;
     int maxBins = 1;
@@ -240,6 +248,8 @@ int finalize_event(tpc_tracker* t) {
                                 cudaMemcpyHostToDevice, t->stream));
     CUDA_TRY(t, cudaMemcpyAsync((void*)t->dev.rowStartBase, t->hostRowStartBase, sizeof(uint32_t) * (t->nRows + 1),
                                 cudaMemcpyHostToDevice, t->stream));
+    CUDA_TRY(t, cudaEventRecord(t->evTables, t->stream));
+    t->tablesPending = true;
     {
         int rc = flush_dirty(t);
         if (rc != TPC_OK) return rc;
@@ -258,16 +268,15 @@ int stage_clusters(tpc_tracker* t, int64_t at, int64_t n, const float* y, const 
         CUDA_TRY(t, cudaMemcpyAsync((float*)t->dev.inY + at, y, sizeof(float) * n, cudaMemcpyDeviceToDevice, t->stream));
         CUDA_TRY(t, cudaMemcpyAsync((float*)t->dev.inZ + at, z, sizeof(float) * n, cudaMemcpyDeviceToDevice, t->stream));
     } else if (n >= (1 << 16) && is_pinned_host_pointer(y) && is_pinned_host_pointer(z)) {
-        // large page-locked buffers: DMA straight from the caller's memory; the call returns when the copy is done,
-        // so the caller may reuse the buffers at once ("copied", tpctrk.h)
+        // large page-locked buffers: DMA straight from the caller's memory.  The call returns when the copy is QUEUED
+        // (DMA || kernels): the caller must not touch the buffers before tpc_wait_input (tpctrk.h)
         int rc = flush_dirty(t);     // keep the order of uploads
         if (rc != TPC_OK) return rc;
         CUDA_TRY(t, cudaMemcpyAsync((float*)t->dev.inY + at, y, sizeof(float) * n, cudaMemcpyHostToDevice, t->stream));
         CUDA_TRY(t, cudaMemcpyAsync((float*)t->dev.inZ + at, z, sizeof(float) * n, cudaMemcpyHostToDevice, t->stream));
         if (!t->evUpload) CUDA_TRY(t, cudaEventCreateWithFlags(&t->evUpload, cudaEventDisableTiming));
         CUDA_TRY(t, cudaEventRecord(t->evUpload, t->stream));
-        CUDA_TRY(t, cudaEventSynchronize(t->evUpload));
-        t->uploadPending = false;
+        t->uploadPending = true;
     } else {
         int rc = ensure_host_stage(t, at + n);
         if (rc != TPC_OK) return rc;
@@ -286,6 +295,46 @@ int stage_clusters(tpc_tracker* t, int64_t at, int64_t n, const float* y, const 
         if (t->dirtyHi == t->dirtyLo) { t->dirtyLo = at; t->dirtyHi = at + n; }
         else t->dirtyHi = at + n;
     }
+    return TPC_OK;
+}
+
+int ensure_out(tpc_tracker* t, int64_t nT, int64_t nC) {
+    if (nT > t->outTracksCap) {
+        tpc_track* nb = nullptr;
+        const int64_t cap = std::max<int64_t>(nT, 1024) * 3 / 2;
+        CUDA_TRY(t, cudaMallocHost(&nb, sizeof(tpc_track) * cap));
+        if (t->outTracks) { CUDA_TRY(t, cudaStreamSynchronize(t->stream)); std::memcpy(nb, t->outTracks, sizeof(tpc_track) * t->outTracksCap); cudaFreeHost(t->outTracks); }
+        t->outTracks = nb; t->outTracksCap = cap;
+    }
+    if (nC > t->outIdsCap) {
+        uint32_t* nb = nullptr;
+        const int64_t cap = std::max<int64_t>(nC, 1024) * 3 / 2;
+        CUDA_TRY(t, cudaMallocHost(&nb, sizeof(uint32_t) * cap));
+        if (t->outIds) { CUDA_TRY(t, cudaStreamSynchronize(t->stream)); std::memcpy(nb, t->outIds, sizeof(uint32_t) * t->outIdsCap); cudaFreeHost(t->outIds); }
+        t->outIds = nb; t->outIdsCap = cap;
+    }
+    return TPC_OK;
+}
+
+// Queue, behind K6, the download of the counters and of the estimated prefix of the result.
+int queue_download(tpc_tracker* t) {
+    cudaStream_t s = t->stream;
+    if (!t->evDone) CUDA_TRY(t, cudaEventCreateWithFlags(&t->evDone, cudaEventDisableTiming));
+    CUDA_TRY(t, cudaMemcpyAsync(t->hostCounters, t->dev.counters, sizeof(uint32_t) * kNCounters, cudaMemcpyDeviceToHost, s));
+    t->queuedTracks = t->queuedIds = 0;
+    if (t->queueOutput && t->nClusters > 0) {
+        // first event: one track per 64 clusters, every cluster in a track; later: the last event's counts + 25 %
+        int64_t eT = t->estTracks > 0 ? t->estTracks : t->nClusters / 64 + 256;
+        int64_t eC = t->estIds > 0 ? t->estIds : t->nClusters;
+        eT = std::min<int64_t>(eT, t->dev.maxTracklets);
+        eC = std::min<int64_t>(eC, t->nClusters);
+        int rc = ensure_out(t, eT, eC);
+        if (rc != TPC_OK) return rc;
+        CUDA_TRY(t, cudaMemcpyAsync(t->outTracks, t->dev.tracks, sizeof(tpc_track) * eT, cudaMemcpyDeviceToHost, s));
+        CUDA_TRY(t, cudaMemcpyAsync(t->outIds, t->dev.clusterIds, sizeof(uint32_t) * eC, cudaMemcpyDeviceToHost, s));
+        t->queuedTracks = eT; t->queuedIds = eC;
+    }
+    CUDA_TRY(t, cudaEventRecord(t->evDone, s));
     return TPC_OK;
 }
 
@@ -402,6 +451,8 @@ void tpc_tracker_destroy(tpc_tracker* t) {
     if (t->outIds) cudaFreeHost(t->outIds);
     if (t->haveEvents) for (auto& e : t->ev) cudaEventDestroy(e);
     if (t->evUpload) cudaEventDestroy(t->evUpload);
+    if (t->evTables) cudaEventDestroy(t->evTables);
+    if (t->evDone) cudaEventDestroy(t->evDone);
     delete t;
 }
 
@@ -414,6 +465,19 @@ int tpc_set_kernel_timing(tpc_tracker* t, int on) {
 int tpc_set_dependent_launch(tpc_tracker* t, int on) {
     if (!t) return TPC_E_ARG;
     t->dependentLaunch = on != 0;
+    return TPC_OK;
+}
+
+int tpc_set_output_prefetch(tpc_tracker* t, int on) {
+    if (!t) return TPC_E_ARG;
+    t->queueOutput = on != 0;
+    return TPC_OK;
+}
+
+int tpc_wait_input(tpc_tracker* t) {
+    if (!t) return TPC_E_ARG;
+    if (t->uploadPending) { CUDA_TRY(t, cudaEventSynchronize(t->evUpload)); t->uploadPending = false; }
+    if (t->tablesPending) { CUDA_TRY(t, cudaEventSynchronize(t->evTables)); t->tablesPending = false; }
     return TPC_OK;
 }
 
@@ -568,6 +632,12 @@ int tpc_track_sectors(tpc_tracker* t) {
     CUDA_TRY(t, launch_dep(pdl, k6_select, 2 * t->k6Blocks, kK6Threads, 0, s, d, dp));   // measured: 2 waves of warps beat 1 here (45 vs 50 us), not in K6a
     CUDA_TRY(t, cudaEventRecord(t->ev[6], s));
     CUDA_TRY(t, cudaGetLastError());
+    // "the tracker can estimate a buffer that is large enough to store all tracks and queue the transfer
+    // of this buffer immediately [...] if the estimation was too small, the tracker can still fetch the rest": the
+    // counters and an estimated prefix of the tracks and cluster ids go to pinned host memory right behind K6, so that
+    // tpc_get_tracks waits once and normally copies nothing.
+    rc = queue_download(t);
+    if (rc != TPC_OK) return rc;
     t->tracked = true; t->fetched = false;
     return TPC_OK;
 }
@@ -577,8 +647,8 @@ int tpc_launches_per_track(const tpc_tracker* t) { (void)t; return 7; }
 int tpc_sync(tpc_tracker* t) {
     if (!t) return TPC_E_ARG;
     if (!t->tracked) return TPC_E_STATE;
-    CUDA_TRY(t, cudaMemcpyAsync(t->hostCounters, t->dev.counters, sizeof(uint32_t) * kNCounters, cudaMemcpyDeviceToHost, t->stream));
-    CUDA_TRY(t, cudaStreamSynchronize(t->stream));
+    CUDA_TRY(t, cudaEventSynchronize(t->evDone));      // K1..K6, the counters and the queued part of the result
+    t->uploadPending = false; t->tablesPending = false;    // (everything queued before it is complete as well)
     std::memcpy(t->counters, t->hostCounters, sizeof(t->counters));
     float total = 0.f;
     for (int i = 0; i < 6; i++) {
@@ -601,19 +671,19 @@ int tpc_get_tracks(tpc_tracker* t, const tpc_track** tracks, int32_t* n_tracks, 
     int rc = tpc_sync(t);
     if (rc != TPC_OK) return rc;
     const int64_t nT = t->counters[kNTracks], nC = t->counters[kNTrackClusters];
-    if (nT > t->outTracksCap) {
-        if (t->outTracks) cudaFreeHost(t->outTracks);
-        t->outTracksCap = std::max<int64_t>(nT, 1024) * 3 / 2;
-        CUDA_TRY(t, cudaMallocHost(&t->outTracks, sizeof(tpc_track) * t->outTracksCap));
+    if (!t->fetched) {
+        // "fetch the rest" only if the queued estimate was short
+        const int64_t haveT = std::min(t->queuedTracks, nT), haveC = std::min(t->queuedIds, nC);
+        if (haveT < nT || haveC < nC) {
+            rc = ensure_out(t, nT, nC);
+            if (rc != TPC_OK) return rc;
+            if (haveT < nT) CUDA_TRY(t, cudaMemcpyAsync(t->outTracks + haveT, t->dev.tracks + haveT, sizeof(tpc_track) * (nT - haveT), cudaMemcpyDeviceToHost, t->stream));
+            if (haveC < nC) CUDA_TRY(t, cudaMemcpyAsync(t->outIds + haveC, t->dev.clusterIds + haveC, sizeof(uint32_t) * (nC - haveC), cudaMemcpyDeviceToHost, t->stream));
+            CUDA_TRY(t, cudaStreamSynchronize(t->stream));
+            t->nRefetch++;
+        }
+        t->estTracks = nT + nT / 4 + 64; t->estIds = nC + nC / 4 + 1024;
     }
-    if (nC > t->outIdsCap) {
-        if (t->outIds) cudaFreeHost(t->outIds);
-        t->outIdsCap = std::max<int64_t>(nC, 1024) * 3 / 2;
-        CUDA_TRY(t, cudaMallocHost(&t->outIds, sizeof(uint32_t) * t->outIdsCap));
-    }
-    if (nT) CUDA_TRY(t, cudaMemcpyAsync(t->outTracks, t->dev.tracks, sizeof(tpc_track) * nT, cudaMemcpyDeviceToHost, t->stream));
-    if (nC) CUDA_TRY(t, cudaMemcpyAsync(t->outIds, t->dev.clusterIds, sizeof(uint32_t) * nC, cudaMemcpyDeviceToHost, t->stream));
-    CUDA_TRY(t, cudaStreamSynchronize(t->stream));
     *tracks = t->outTracks; *n_tracks = (int32_t)nT; *cluster_ids = t->outIds; *n_cluster_ids = nC;
     t->fetched = true;
     return t->counters[kNStart] > (uint32_t)t->dev.maxTracklets ? TPC_E_OVERFLOW : TPC_OK;
@@ -626,6 +696,7 @@ int tpc_get_stats(tpc_tracker* t, tpc_stats* out) {
     out->max_clusters = t->maxClusters;
     out->max_tracklets = t->ws ? t->dev.maxTracklets : 0;
     out->workspace_bytes_used = (int64_t)t->L.total;
+    out->n_output_refetches = t->nRefetch;
     if (!t->tracked) return TPC_OK;
     out->n_links = t->counters[kNLinks];
     out->n_start_hits = t->counters[kNStart];

@@ -294,7 +294,7 @@ def test_several_events_per_call_as_extra_sectors():
 
 def test_page_locked_host_input_is_read_directly():
     """Large page-locked host buffers are uploaded straight from the caller's memory (no staging copy); the call
-    returns after the copy, so the buffers may be overwritten at once."""
+    returns when the copy is queued, tpc_wait_input when the buffers may be overwritten."""
     torch = _cuda()
     ev = datagen.config_event(2, seed=9)
     ref = oracle.run_event(ev)
@@ -302,7 +302,8 @@ def test_page_locked_host_input_is_read_directly():
     trk.set_stream(torch.cuda.current_stream().cuda_stream)
     trk.allocate_workspace(ev.n_clusters)
     y, z = torch.from_numpy(ev.y.copy()).pin_memory(), torch.from_numpy(ev.z.copy()).pin_memory()
-    trk.load_event(ev.row_counts, y.numpy(), z.numpy())
+    trk.load_event(ev.row_counts, y.numpy(), z.numpy())    # returns when the copy is queued (tpctrk.h)
+    trk.wait_input()                                       # ... and this when it has been read
     y.fill_(float("nan")); z.fill_(float("nan"))          # must not matter any more
     trk.track_sectors()
     tracks, ids = trk.get_tracks()
@@ -592,3 +593,32 @@ def test_reloading_rows_in_place_does_not_use_up_the_staging_area():
     trk.track_sectors()
     tracks, ids = trk.get_tracks()
     compare(ev, trk, tracks, ids, ref)
+
+
+def test_queued_download_and_fetching_the_rest():
+    """the download of an estimated part of the result is queued behind the kernels; "if the estimation
+    was too small, the tracker can still fetch the rest".  A small event first (its counts become the estimate), then a
+    large one: tpc_get_tracks must fetch the remainder (counted in the stats) and the result must equal the oracle's;
+    the large event again: the estimate now covers it, no further fetch.  With the prefetch off the result is the same."""
+    torch = _cuda()
+    small, big = datagen.config_event(1, seed=30), datagen.config_event(2, seed=31)
+    ref_small, ref_big = oracle.run_event(small), oracle.run_event(big)
+    trk = binding.Tracker(big.n_sectors, big.n_rows, big.row_x, big.bz)
+    trk.set_stream(torch.cuda.current_stream().cuda_stream)
+    trk.allocate_workspace(big.n_clusters)
+    _, tracks, ids = run_gpu(small, tracker=trk)
+    compare(small, trk, tracks, ids, ref_small)
+    assert trk.get_stats()["n_output_refetches"] == 0          # first estimate: N/64 tracks, N ids - enough
+    _, tracks, ids = run_gpu(big, tracker=trk)
+    assert trk.get_stats()["n_output_refetches"] == 1          # estimate came from the small event: the rest was fetched
+    out = compare(big, trk, tracks, ids, ref_big)
+    assert out["tracklet_mismatch"] == 0
+    t_again, i_again = trk.get_tracks()                          # asking again neither copies nor changes anything
+    assert np.array_equal(i_again, ids) and trk.get_stats()["n_output_refetches"] == 1
+    _, tracks, ids = run_gpu(big, tracker=trk)
+    assert trk.get_stats()["n_output_refetches"] == 1
+    compare(big, trk, tracks, ids, ref_big)
+    trk.set_output_prefetch(False)
+    _, tracks, ids = run_gpu(big, tracker=trk)
+    assert trk.get_stats()["n_output_refetches"] == 2          # nothing was queued: everything is "the rest"
+    compare(big, trk, tracks, ids, ref_big)
