@@ -44,6 +44,63 @@ def algorithmic_bytes(st: dict) -> dict:
     }
 
 
+def source_sha16() -> str:
+    """Hash of the CUDA sources the library is built from: ties profiles/kernel_counters.json to a build."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_1712_09430_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh")):
+            h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:16]
+
+
+COUNTERS = os.path.join(ROOT, "profiles", "kernel_counters.json")
+NCU_KERNELS = {"K1_sort_grid": "k1_sort_grid", "K2_neighbours": "k2_neighbours", "K3K4_clean_start": "k3_clean_start",
+               "K5_construct": "k5_construct_phased", "K6a_weights": "k6_weights", "K6b_select": "k6_select"}
+
+
+def ncu_summary(rep: str):
+    """`bench.py --ncu-summary REPORT.ncu-rep`: per-kernel counters of one `ncu --set full` capture of bench.py ->
+    profiles/kernel_counters.json (instructions, DRAM bytes, lanes per instruction), stamped with the hash of the CUDA
+    sources.  bench.py quotes them (roofline.traffic, roofline_issue) only while that hash is the current one."""
+    import csv
+    import subprocess
+    raw = subprocess.run(["ncu", "-i", rep, "--page", "raw", "--csv"], capture_output=True, text=True, check=True).stdout
+    rows = list(csv.reader(raw.splitlines()))
+    hdr = rows[0]
+    col = {h: i for i, h in enumerate(hdr)}
+    units = rows[1]
+    out = {"source_sha16": source_sha16(), "report": os.path.basename(rep), "kernels": {}}
+    for key, name in NCU_KERNELS.items():
+        for r in rows[2:]:
+            if name in r[col["Kernel Name"]]:
+                def val(m, scale_bytes=False):
+                    v = float(r[col[m]].replace(",", ""))
+                    if scale_bytes:
+                        v *= {"byte": 1, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}[units[col[m]]]
+                    return v
+                out["kernels"][key] = {
+                    "inst_executed": int(val("smsp__inst_executed.sum")),
+                    "threads_per_inst": round(val("smsp__thread_inst_executed_per_inst_executed.ratio"), 2),
+                    "dram_bytes": int(val("dram__bytes_read.sum", True) + val("dram__bytes_write.sum", True)),
+                    "ncu_us": round(val("gpu__time_duration.sum"), 2),
+                    "warps_per_scheduler": round(val("smsp__warps_active.avg.per_cycle_active"), 2),
+                }
+                break
+    json.dump(out, open(COUNTERS, "w"), indent=1)
+    print(json.dumps(out))
+
+
+def kernel_counters():
+    """profiles/kernel_counters.json if it describes the current sources, else None (never a stale number)."""
+    try:
+        c = json.load(open(COUNTERS))
+        return c if c.get("source_sha16") == source_sha16() else None
+    except Exception:
+        return None
+
+
 def measured_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -159,6 +216,10 @@ def oracle_baseline(ev, budget_s: float = 15.0):
         best = min(best, time.perf_counter() - t0)
     out = {"value": sample.n_clusters / best, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc,
            "seconds": best, "stage_seconds": o.stage_seconds()}
+    # north_star: decisions the oracle's own candidates tie within 1e-6 relative are "counted and reported"
+    res = o.fetch()
+    out["near_ties"] = {"s2_hits": int(res.tie_s2.sum()), "tracklets": int(res.tracklets["near_tie"].sum()),
+                        "of_hits": int(res.n_clusters), "of_tracklets": int(res.tracklets.size)}
     # the SAME single-threaded oracle, one instance per sector, on a pool of P host
     # threads (sectors are independent; ctypes releases the GIL).  Context next to the 1-core number.
     try:
@@ -195,6 +256,7 @@ def multi_event_leg(torch, binding, datagen, args, params, dev, rank: int, k: in
     y = torch.from_numpy(np.concatenate([e.y for e in evs])).to(dev)
     z = torch.from_numpy(np.concatenate([e.z for e in evs])).to(dev)
     trk.load_event(counts, y, z)
+    trk.set_output_prefetch(False)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
     times = []
     for i in range(3 + reps):
@@ -217,6 +279,41 @@ def multi_event_leg(torch, binding, datagen, args, params, dev, rank: int, k: in
             "value": n_total / (ms * 1e-3), "unit": UNIT, "n_tracks": st["n_tracks"],
             "kernel_us_per_event": {kk: round(v / k, 1) for kk, v in st["kernel_us"].items()},
             "note": "k independent synthetic events (other seeds) as 36*k sectors of one tracker, one call"}
+
+
+def time_frame_leg(torch, binding, datagen, params, dev, reps: int = 3):
+    """BASELINE.json:configs[4] (extra key, not the headline): a Run-3-style time frame - 20 overlapped central events,
+    ~31.6 M clusters - tracked by ONE tpc_track_sectors call (north_star).  Same timing rules as the main leg."""
+    ev = datagen.config_event(4, seed=0)
+    trk = binding.Tracker(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz, params)
+    stream = torch.cuda.current_stream()
+    trk.set_stream(stream.cuda_stream)
+    ws = trk.allocate_workspace(ev.n_clusters, device=dev)
+    trk.load_event(ev.row_counts, torch.from_numpy(ev.y).to(dev), torch.from_numpy(ev.z).to(dev))
+    trk.set_output_prefetch(False)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    times = []
+    for i in range(1 + reps):
+        flush.fill_(1)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        trk.track_sectors()
+        b.record(stream)
+        trk.sync()
+        if i >= 1:
+            times.append(a.elapsed_time(b))
+    ms = sum(times) / len(times)
+    trk.set_kernel_timing(True)
+    flush.fill_(1)
+    trk.track_sectors()
+    trk.sync()
+    st = trk.get_stats()
+    trk.destroy()
+    return {"workload": "config4:timeframe-20x-central", "n_clusters": ev.n_clusters, "calls": reps, "ms_per_call": ms,
+            "value": ev.n_clusters / (ms * 1e-3), "unit": UNIT, "central_events_per_sec": 20.0 / (ms * 1e-3),
+            "n_start_hits": st["n_start_hits"], "n_tracklet_hits": st["n_tracklet_hits"], "n_tracks": st["n_tracks"],
+            "workspace_over_input": round(ws / (12.0 * ev.n_clusters), 2),
+            "kernel_us": {k: round(v, 1) for k, v in st["kernel_us"].items()}}
 
 
 def run_reference(args, rank, world, dist):
@@ -263,11 +360,17 @@ def main():
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--e2e-instances", type=int, default=4, help="tracker instances / host threads / streams of the end-to-end leg")
+    ap.add_argument("--e2e-instances", type=int, default=3, help="tracker instances (streams) the ONE host thread of the end-to-end leg keeps in flight")
+    ap.add_argument("--no-time-frame", action="store_true", help="skip the configs[4] leg (20 overlapped central events in one call)")
+    ap.add_argument("--ncu-summary", default=None, metavar="REPORT.ncu-rep",
+                    help="no benchmark: extract per-kernel counters of an ncu capture of bench.py into profiles/kernel_counters.json")
     ap.add_argument("--bins-per-hit", type=float, default=None, help="override tpc_params.grid_bins_per_hit (tuning)")
     ap.add_argument("--events-per-call", type=int, default=4,
                     help="extra leg: this many events tracked by one call (PAPER.md:82-84); 0 or 1 = skip")
     args = ap.parse_args()
+    if args.ncu_summary:
+        ncu_summary(args.ncu_summary)
+        return
     rank, world, local, dist = init_dist(args.gpus)
     if args.impl == "reference":
         run_reference(args, rank, world, dist)
@@ -295,6 +398,7 @@ def main():
     ws_bytes = trk.allocate_workspace(ev.n_clusters, device=dev)
     y_dev, z_dev = torch.from_numpy(ev.y).to(dev), torch.from_numpy(ev.z).to(dev)
     trk.load_event(ev.row_counts, y_dev, z_dev)          # inputs resident in HBM before the timed region
+    trk.set_output_prefetch(False)                       # device-timed leg: K1..K6 only (no result download queued behind K6)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
 
     def step_device():
@@ -347,51 +451,49 @@ def main():
     value, ms, n_total = aggregate(dist, dev, ev.n_clusters, step_ms)
 
     # ---- end to end through the C ABI with HOST buffers (pinned), H2D + D2H of every step inside the timed region.
-    # Four tracker instances, each driven by its own host thread on its own stream, take events in turn: while one
-    # tracks, the others upload their next event / download their tracks (the paper's DMA || kernel pipeline,
-    # PAPER.md:66 and Fig. 4).  Every step still does load_event (pinned host -> device), track_sectors, get_tracks
-    # (device -> pinned host); time = wall clock around all steps of both threads.
-    n_pipe = max(1, args.e2e_instances)      # measured on config 3, two boxes: 2 / 3 / 4 instances -> 0.99 / 0.76 / 0.84 and 1.25 / 1.03 / 0.78 ms per event
+    # ONE host thread keeps n_pipe tracker instances (each on its own stream) in flight, round robin: for the oldest
+    # instance tpc_get_tracks (waits once: the download was queued behind its kernels), then
+    # tpc_load_event (page-locked input, returns when the copy is queued) and tpc_track_sectors for its next event -
+    # the paper's DMA || kernels pipeline (Fig. 4) with several tracker instances per GPU.
+    n_pipe = max(1, args.e2e_instances)
     pipes = []
     for i in range(n_pipe):
         sti = torch.cuda.Stream(device=dev)
-        ti = trk if i == 0 else binding.Tracker(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz, params)
-        if i > 0:
-            ti.set_stream(sti.cuda_stream)
-            ti.allocate_workspace(ev.n_clusters, device=dev)
-        pipes.append((ti, torch.from_numpy(ev.y.copy()).pin_memory(), torch.from_numpy(ev.z.copy()).pin_memory()))
-    if n_pipe > 1:
-        for ti, _, _ in pipes:
+        ti = binding.Tracker(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz, params)
+        ti.set_stream(sti.cuda_stream)
+        ti.allocate_workspace(ev.n_clusters, device=dev)
+        if n_pipe > 1:
             ti.set_dependent_launch(False)     # several trackers on concurrent streams: ordinary launches (tpctrk.h)
-    last = [None] * n_pipe
+        pipes.append((ti, sti, torch.from_numpy(ev.y.copy()).pin_memory(), torch.from_numpy(ev.z.copy()).pin_memory()))
+    last = [None]
 
-    def e2e_worker(i, n):
-        torch.cuda.set_device(dev)
-        ti, yp, zp = pipes[i]
-        for _ in range(n):
-            ti.load_event(ev.row_counts, yp.numpy(), zp.numpy())
-            ti.track_sectors()
-            last[i] = ti.get_tracks(copy=False)
-
-    def e2e_run(n_each):
-        ths = [threading.Thread(target=e2e_worker, args=(i, n_each)) for i in range(n_pipe)]
+    def e2e_run(n_events):
+        """n_events events through the n_pipe instances; returns wall seconds."""
+        torch.cuda.synchronize()
         t0 = time.perf_counter()
-        for th in ths:
-            th.start()
-        for th in ths:
-            th.join()
+        for i in range(n_events + n_pipe):
+            ti, _, yp, zp = pipes[i % n_pipe]
+            if i >= n_pipe:
+                last[0] = ti.get_tracks(copy=False)          # result of event i - n_pipe
+            if i < n_events:
+                ti.load_event(ev.row_counts, yp.numpy(), zp.numpy())
+                ti.track_sectors()
         torch.cuda.synchronize()
         return time.perf_counter() - t0
 
-    e2e_run(2)
+    e2e_run(2 * n_pipe)
     if dist is not None:
         dist.barrier()
-    n_e2e = max(8, min(4 * args.steps, 96)) // n_pipe * n_pipe     # ~60 ms of wall clock: thread start-up is noise below that
-    e2e_ms = e2e_run(n_e2e // n_pipe) / n_e2e * 1e3
+    n_e2e = max(12, min(4 * args.steps, 96)) // n_pipe * n_pipe
+    e2e_ms = e2e_run(n_e2e) / n_e2e * 1e3
     tr, ids = last[0]
     e2e_value, e2e_ms_max, _ = aggregate(dist, dev, ev.n_clusters, e2e_ms)
     h2d = 8 * ev.n_clusters + 48 * ev.n_sectors * ev.n_rows + 4 * (ev.n_sectors + 1)
-    d2h = 112 * int(tr.shape[0]) + 4 * int(ids.shape[0]) + 64
+    est_t, est_c = int(tr.shape[0]) + int(tr.shape[0]) // 4 + 64, int(ids.shape[0]) + int(ids.shape[0]) // 4 + 1024
+    d2h = 112 * est_t + 4 * min(est_c, ev.n_clusters) + 64           # what is queued: the estimate (counts + 25 %), not the exact size
+    e2e_refetches = sum(p[0].get_stats()["n_output_refetches"] for p in pipes)
+    for p_ in pipes:
+        p_[0].destroy()
 
     # ---- roofline of the dominant kernel + per-kernel table
     peak, peak_src = measured_peaks()
@@ -404,13 +506,24 @@ def main():
     per_kernel = {k: {"us": round(kern[k], 2), "alg_bytes": ab[k], "gbs": round(ab[k] / (kern[k] * 1e-6) / 1e9, 1),
                       "frac": round(ab[k] / (kern[k] * 1e-6) / 1e9 / peak, 4)} for k in kern}
     achieved = ab[dom] / (kern[dom] * 1e-6) / 1e9
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", "dominant_kernel_traffic.json")
-    if os.path.exists(tp):
-        try:
-            traffic = json.load(open(tp)).get(dom)
-        except Exception:
-            traffic = None
+    # counters of an ncu capture of THIS build (profiles/kernel_counters.json carries the hash of the CUDA sources;
+    # with other sources the file is ignored: no stale number)
+    cnt = kernel_counters()
+    traffic = cnt["kernels"].get(dom, {}).get("dram_bytes") if cnt else None
+    # What bounds these kernels is instruction issue and latency, not HBM: issue roofline =
+    # warp instructions executed (ncu smsp__inst_executed.sum of the same build) / CUDA-event time, against the peak of
+    # one instruction per cycle and scheduler: SMs x 4 x the SM clock sampled during the timed region.
+    roof_issue = None
+    if cnt and clocks.get("sm_mhz"):
+        sms = torch.cuda.get_device_properties(dev).multi_processor_count
+        peak_ips = sms * 4 * clocks["sm_mhz"] * 1e6
+        roof_issue = {"unit": "warp-inst/s", "peak": peak_ips, "peak_source": f"{sms} SMs x 4 schedulers x {clocks['sm_mhz']} MHz (sampled)",
+                      "counters": "profiles/kernel_counters.json (ncu, same CUDA sources)", "kernels": {}}
+        for k in kern:
+            c = cnt["kernels"].get(k)
+            if c and kern[k] > 0:
+                roof_issue["kernels"][k] = {"inst": c["inst_executed"], "frac": round(c["inst_executed"] / (kern[k] * 1e-6) / peak_ips, 4),
+                                            "threads_per_inst": c["threads_per_inst"], "warps_per_scheduler": c["warps_per_scheduler"]}
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "warmup_actual": n_warm, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -426,8 +539,9 @@ def main():
                    "kernel_times": "second pass of the same K steps with a CUDA event between the kernels (tpc_set_kernel_timing)"},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms_max, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "steps": n_e2e, "pipeline": f"{n_pipe} tracker instances / host threads / streams: copies of one event overlap the kernels of the others; ordinary (not dependent) launches"},
-        "gpu_launches": args.steps * trk.launches_per_track(),
+                "steps": n_e2e, "output_refetches": e2e_refetches,
+                "pipeline": f"one host thread, {n_pipe} tracker instances (streams) in flight: page-locked input read by DMA without blocking, result download queued behind K6 (estimate = last counts + 25 %), one wait per event"},
+        "gpu_launches": 2 * args.steps * trk.launches_per_track(),      # the K timed steps and their second pass with kernel timing
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": round(achieved, 2), "peak": peak, "unit": "GB/s",
                      "frac": round(achieved / peak, 5), "traffic": traffic, "peak_source": peak_src,
                      "frac_of_8TBs_nominal": round(achieved / 8000.0, 5),
@@ -435,12 +549,18 @@ def main():
                                     "frac": round(sum(ab.values()) / (ms * 1e-3) / 1e9 / peak, 5)}},
         "kernels": per_kernel,
     }
+    if roof_issue:
+        out["roofline_issue"] = roof_issue
     if args.events_per_call > 1 and args.config <= 3:
         me = multi_event_leg(torch, binding, datagen, args, params, dev, rank, args.events_per_call, max(3, min(args.steps, 10)))
         me["value"] = reduce_over_ranks(dist, me["value"], "sum", dev)      # whole job: sum of the ranks' rates
         out["multi_event"] = me
+    if rank == 0 and not args.no_time_frame and args.config == 3:
+        del trk, y_dev, z_dev                            # (the time frame needs ~9 GB of workspace)
+        out["time_frame"] = time_frame_leg(torch, binding, datagen, params, dev)
     if rank == 0 and not args.no_cpu_baseline:
         out["cpu_baseline"] = oracle_baseline(datagen.config_event(args.config, seed=0))
+        out["config"]["near_ties"] = out["cpu_baseline"].get("near_ties")
     if dist is not None:
         dist.barrier()
     if rank == 0:
