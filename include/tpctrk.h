@@ -55,9 +55,9 @@ typedef struct tpc_params {
     int32_t max_gap;                /* a leg stops at the (max_gap+1)-th consecutive empty row              4 */
     int32_t min_hits;               /* min hits of a kept tracklet and min owned hits of a track           10 */
     int32_t seed_min_chain;         /* min link-chain length of a seed ("3 to about 10")        3 */
-    float max_tracklets_per_cluster;/* capacity estimate for tracklets                    0.125 */
+    float max_tracklets_per_cluster;/* capacity estimate for tracklets                      0.1 */
     float grid_bins_per_hit;        /* resolution of the per-row y/z grid (accelerator only: no result
-                                       depends on it), bins per cluster of the row, 0.25..64                3 */
+                                       depends on it), bins per cluster of the row, 0.25..64                2 */
 } tpc_params;
 
 typedef struct tpc_geometry {

@@ -401,8 +401,8 @@ void tpc_default_params(tpc_params* p) {
     p->kf_css0 = 1.0f; p->kf_ctt0 = 10.0f; p->kf_ckk0 = 100.0f; p->kf_smax = 0.95f;
     p->road_nsig = 4.0f; p->road_max = 2.0f;
     p->max_gap = 4; p->min_hits = 10; p->seed_min_chain = 3;
-    p->max_tracklets_per_cluster = 0.125f;
-    p->grid_bins_per_hit = 3.0f;
+    p->max_tracklets_per_cluster = 0.1f;
+    p->grid_bins_per_hit = 2.0f;
 }
 
 int tpc_tracker_create(const tpc_geometry* g, float bz_tesla, tpc_tracker** out) {
