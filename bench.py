@@ -361,6 +361,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-instances", type=int, default=3, help="tracker instances (streams) the ONE host thread of the end-to-end leg keeps in flight")
+    ap.add_argument("--neighbour-staging", action="store_true", help="K2 with its neighbour rows staged in shared memory (tpc_set_neighbour_staging; slower, for the ncu comparison)")
     ap.add_argument("--no-time-frame", action="store_true", help="skip the configs[4] leg (20 overlapped central events in one call)")
     ap.add_argument("--ncu-summary", default=None, metavar="REPORT.ncu-rep",
                     help="no benchmark: extract per-kernel counters of an ncu capture of bench.py into profiles/kernel_counters.json")
@@ -399,6 +400,7 @@ def main():
     y_dev, z_dev = torch.from_numpy(ev.y).to(dev), torch.from_numpy(ev.z).to(dev)
     trk.load_event(ev.row_counts, y_dev, z_dev)          # inputs resident in HBM before the timed region
     trk.set_output_prefetch(False)                       # device-timed leg: K1..K6 only (no result download queued behind K6)
+    trk.set_neighbour_staging(args.neighbour_staging)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
 
     def step_device():

@@ -135,6 +135,12 @@ int tpc_set_kernel_timing(tpc_tracker* t, int on);
  * better: measured 0.73 vs 0.87 ms per event with four trackers in flight; switch it off there. */
 int tpc_set_dependent_launch(tpc_tracker* t, int on);
 
+/* on != 0: the neighbours finder (K2) stages the pieces of the two adjacent pad rows that a block's hits can reach
+ * in shared memory (bulk copies by the TMA engine) before it scans them; off (default): it reads them through L1.
+ * A launch option like the two above: results are identical.  Off is faster on B200 for every workload measured
+ * (central event 90 vs 120 us, time frame 10.0 vs 11.4 ms; profiles/r02_k2_staging.md). */
+int tpc_set_neighbour_staging(tpc_tracker* t, int on);
+
 /* Device bytes needed for events of up to max_clusters clusters (internal buffers). */
 size_t tpc_workspace_bytes(const tpc_tracker* t, int64_t max_clusters);
 /* dev_ptr: device pointer, 256-byte aligned, caller-owned, must outlive its use.  Capacity is derived from bytes. */

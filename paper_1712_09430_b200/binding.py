@@ -82,6 +82,7 @@ def lib():
         L.tpc_set_kernel_timing.argtypes = [vp, ctypes.c_int]
         L.tpc_set_dependent_launch.argtypes = [vp, ctypes.c_int]
         L.tpc_set_output_prefetch.argtypes = [vp, ctypes.c_int]
+        L.tpc_set_neighbour_staging.argtypes = [vp, ctypes.c_int]
         L.tpc_wait_input.argtypes = [vp]
         L.tpc_workspace_bytes.argtypes = [vp, i64]
         L.tpc_workspace_bytes.restype = ctypes.c_size_t
@@ -169,6 +170,9 @@ class Tracker:
 
     def set_dependent_launch(self, on: bool):
         self._check(self._L.tpc_set_dependent_launch(self._h, 1 if on else 0), "tpc_set_dependent_launch")
+
+    def set_neighbour_staging(self, on: bool):
+        self._check(self._L.tpc_set_neighbour_staging(self._h, 1 if on else 0), "tpc_set_neighbour_staging")
 
     def set_output_prefetch(self, on: bool):
         self._check(self._L.tpc_set_output_prefetch(self._h, 1 if on else 0), "tpc_set_output_prefetch")

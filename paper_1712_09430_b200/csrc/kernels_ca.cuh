@@ -251,7 +251,21 @@ __device__ __forceinline__ void scan_ranges(const WinRanges& w, const RowGrid& R
 }
 
 // ------------------------------------------------------------------------------------------ K2
-// Neighbours finder (S2): for each hit the best (up,down) pair in rows r+1/r-1 by 3-point collinearity.
+// Neighbours finder (S2): for each hit the best (up,down) pair in rows r+1/r-1 by 3-point collinearity; one thread
+// per hit.
+//
+// A block takes a CHUNK of up to kK2Chunk consecutive sorted hits of one (sector,row) (a row of a time frame holds
+// ~5,500 hits: one block per row left most SMs waiting for the longest rows, 15.3 -> 10.0 ms for K2 there).  K1 sorted
+// the hits by bin, z-major, so a chunk covers a band in z, and everything its hits can reach in an adjacent row - the
+// rows of bins that overlap [zmin - window, zmax + window] - is ONE contiguous piece of that row's sorted hits and of
+// its bin table.
+// kStage (tpc_set_neighbour_staging, OFF by default): those two pieces per adjacent row are staged in shared memory
+// first, the hits with a 1-D bulk copy (cp.async.bulk + mbarrier: the TMA engine), the bin table with coalesced
+// loads; every candidate scan then reads shared memory.  A piece that does not fit (kK2StageHits / kK2StageBins)
+// makes the block read global memory like the unstaged instantiation (same code, other pointers).  Measured, it
+// loses: 120 vs 90 us on a central event, 11.4 vs 10.0 ms on a time frame - a block's work is a few microseconds
+// (2-3 hits per thread), and the z-band pass, the barrier and the wait for the copies stand in front of all of it,
+// while the unstaged scans already hit L1 for 77 % of their sectors (profiles/r02_k2_staging.md has both columns).
 #ifndef TPC_K2T
 #define TPC_K2T 128
 #endif
@@ -260,16 +274,95 @@ constexpr int kK2Threads = TPC_K2T;
 #define TPC_K2CAP 8
 #endif
 constexpr int kK2Cap = TPC_K2CAP;   // down-candidates cached per thread; beyond that a nested rescan (slow, exact)
-
 #ifndef TPC_K2B
 #define TPC_K2B 8
 #endif
+#ifndef TPC_K2CHUNK
+#define TPC_K2CHUNK 256   /* 128 / 256 / 512 / 1024: K2 90.8 / 89.5 / 91.7 / 91.5 us (central event), 10.2 / 9.9 / 10.0 / 10.6 ms (time frame) */
+#endif
+constexpr int kK2Chunk = TPC_K2CHUNK;
+constexpr int kK2StageHits = 1024;      // staged hits of each adjacent row (8 KB)
+constexpr int kK2StageBins = 1280;      // staged bin-table entries of each adjacent row (5 KB)
+
+// One adjacent row as the scans see it: hs[k - kBase] is sorted hit k, bs[b - bBase] is bin-table entry b.
+struct K2Row {
+    const float2* hs;
+    const uint32_t* bs;
+    int kBase, bBase;
+};
+__device__ __forceinline__ WinRanges k2_win_ranges(const RowGrid& R, const K2Row& V, float yc, float zc, float wy, float wz) {
+    WinRanges w;
+    w.by0 = bin_of(yc - wy - kGridMargin, R.y0, R.invY, R.nY);
+    w.by1 = bin_of(yc + wy + kGridMargin, R.y0, R.invY, R.nY);
+    w.bz0 = bin_of(zc - wz - kGridMargin, R.z0, R.invZ, R.nZ);
+    w.bz1 = bin_of(zc + wz + kGridMargin, R.z0, R.invZ, R.nZ);
+    const uint32_t* __restrict__ bs = V.bs - V.bBase;
+#pragma unroll
+    for (int j = 0; j < 3; j++) {
+        const int bz = min(w.bz0 + j, w.bz1);           // rows beyond the window repeat the last one (valid address)
+        const bool in = w.bz0 + j <= w.bz1;
+        const int a = (int)bs[bz * R.nY + w.by0], b = (int)bs[bz * R.nY + w.by1 + 1];
+        w.k0[j] = in ? a : 0;
+        w.k1[j] = in ? b : 0;
+    }
+    return w;
+}
+template <class F>
+__device__ __forceinline__ void k2_scan(const WinRanges& w, const RowGrid& R, const K2Row& V, F&& f) {
+    const float2* __restrict__ hs = V.hs - V.kBase;
+    if (w.bz1 - w.bz0 <= 2) {
+        // one loop over the three ranges laid end to end: the warp runs max over lanes of the TOTAL length, not the
+        // sum over ranges of the per-range maxima
+        const int l0 = w.k1[0] - w.k0[0], l1 = l0 + (w.k1[1] - w.k0[1]), l2 = l1 + (w.k1[2] - w.k0[2]);
+        const int o1 = w.k0[1] - l0, o2 = w.k0[2] - l1;
+        auto at = [&](int t) { return t < l0 ? w.k0[0] + t : t < l1 ? o1 + t : o2 + t; };
+        if (l2 > 0) {
+            int k = at(0);
+            float2 c = hs[k];
+            for (int t = 0; t < l2; t++) {
+                const int kn = at(min(t + 1, l2 - 1));      // next candidate requested before this one is examined
+                const float2 cn = hs[kn];
+                f(k, c);
+                k = kn; c = cn;
+            }
+        }
+    } else {
+        const uint32_t* __restrict__ bs = V.bs - V.bBase;
+        for (int bz = w.bz0; bz <= w.bz1; bz++) {
+            const int k0 = (int)bs[bz * R.nY + w.by0], k1 = (int)bs[bz * R.nY + w.by1 + 1];
+            for (int k = k0; k < k1; k++) f(k, hs[k]);
+        }
+    }
+}
+template <class F>
+__device__ __forceinline__ void k2_for_window(const RowGrid& R, const K2Row& V, float yc, float zc, float wy, float wz, F&& f) {
+    const int by0 = bin_of(yc - wy - kGridMargin, R.y0, R.invY, R.nY);
+    const int by1 = bin_of(yc + wy + kGridMargin, R.y0, R.invY, R.nY);
+    const int bz0 = bin_of(zc - wz - kGridMargin, R.z0, R.invZ, R.nZ);
+    const int bz1 = bin_of(zc + wz + kGridMargin, R.z0, R.invZ, R.nZ);
+    const uint32_t* __restrict__ bs = V.bs - V.bBase;
+    const float2* __restrict__ hs = V.hs - V.kBase;
+    for (int bz = bz0; bz <= bz1; bz++) {
+        const int k0 = (int)bs[bz * R.nY + by0], k1 = (int)bs[bz * R.nY + by1 + 1];
+        for (int k = k0; k < k1; k++) f(k, hs[k]);
+    }
+}
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+template <bool kStage>
 __global__ void __launch_bounds__(kK2Threads, TPC_K2B) k2_neighbours(DevPtrs d, DevParams dp) {
+    __shared__ __align__(16) float2 sHitsU[kStage ? kK2StageHits : 1], sHitsD[kStage ? kK2StageHits : 1];
+    __shared__ uint32_t sBinsU[kStage ? kK2StageBins : 1], sBinsD[kStage ? kK2StageBins : 1];
+    __shared__ __align__(8) unsigned long long sBar;
+    __shared__ float sRedLo[kK2Threads / 32], sRedHi[kK2Threads / 32];
     grid_dep_wait();
     const int rowId = blockIdx.x;
     const int r = rowId % dp.nRows;
     const int n = d.meta[rowId].n;
-    if (n == 0) return;
+    const int i0 = blockIdx.y * kK2Chunk;
+    if (i0 >= n) return;
+    const int i1 = min(n, i0 + kK2Chunk);
     const RowGrid R = d.grid[rowId];
     int32_t* __restrict__ up = d.linkUp + R.hitOff;
     int32_t* __restrict__ dn = d.linkDn + R.hitOff;
@@ -280,7 +373,7 @@ __global__ void __launch_bounds__(kK2Threads, TPC_K2B) k2_neighbours(DevPtrs d, 
         active = d.meta[rowId + 1].n > 0 && d.meta[rowId - 1].n > 0;
     }
     if (!active) {
-        for (int i = threadIdx.x; i < n; i += kK2Threads) { up[i] = -1; dn[i] = -1; }
+        for (int i = i0 + threadIdx.x; i < i1; i += kK2Threads) { up[i] = -1; dn[i] = -1; }
         return;
     }
     const float xr = d.rowX[r];
@@ -291,15 +384,70 @@ __global__ void __launch_bounds__(kK2Threads, TPC_K2B) k2_neighbours(DevPtrs d, 
     const float wyD = dp.P.nf_ty * (-dxd) + dp.P.nf_c, wzD = dp.P.nf_tz * (-dxd) + dp.P.nf_c;
     const uint32_t* __restrict__ origU = d.orig + Ru.hitOff;
     const uint32_t* __restrict__ origD = d.orig + Rd.hitOff;
+    K2Row VU{d.hits + Ru.hitOff, d.binStart + Ru.binOff, 0, 0}, VD{d.hits + Rd.hitOff, d.binStart + Rd.binOff, 0, 0};
 
-    for (int i = threadIdx.x; i < n; i += kK2Threads) {
+    if constexpr (kStage) {
+        // z band of the chunk (its hits are read again below: L1)
+        float zlo = 3.0e38f, zhi = -3.0e38f;
+        for (int i = i0 + threadIdx.x; i < i1; i += kK2Threads) {
+            const float z = d.hits[R.hitOff + i].y;
+            zlo = fminf(zlo, z); zhi = fmaxf(zhi, z);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            zlo = fminf(zlo, __shfl_xor_sync(0xffffffffu, zlo, o));
+            zhi = fmaxf(zhi, __shfl_xor_sync(0xffffffffu, zhi, o));
+        }
+        if ((threadIdx.x & 31) == 0) { sRedLo[threadIdx.x >> 5] = zlo; sRedHi[threadIdx.x >> 5] = zhi; }
+        if (threadIdx.x == 0) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&sBar)));
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        }
+        __syncthreads();
+#pragma unroll
+        for (int w = 0; w < kK2Threads / 32; w++) { zlo = fminf(zlo, sRedLo[w]); zhi = fmaxf(zhi, sRedHi[w]); }
+        // the pieces: rows of bins [bLo, bHi] of each neighbour, hits [k0, k1)
+        const int uLo = bin_of(zlo - wzU - kGridMargin, Ru.z0, Ru.invZ, Ru.nZ), uHi = bin_of(zhi + wzU + kGridMargin, Ru.z0, Ru.invZ, Ru.nZ);
+        const int dLo = bin_of(zlo - wzD - kGridMargin, Rd.z0, Rd.invZ, Rd.nZ), dHi = bin_of(zhi + wzD + kGridMargin, Rd.z0, Rd.invZ, Rd.nZ);
+        const int ubBase = uLo * Ru.nY, ubCnt = (uHi - uLo + 1) * Ru.nY + 1;
+        const int dbBase = dLo * Rd.nY, dbCnt = (dHi - dLo + 1) * Rd.nY + 1;
+        const int uk0 = (int)VU.bs[ubBase] & ~1, uk1 = (int)VU.bs[ubBase + ubCnt - 1];      // (16-byte aligned start)
+        const int dk0 = (int)VD.bs[dbBase] & ~1, dk1 = (int)VD.bs[dbBase + dbCnt - 1];
+        const int uLen = (uk1 - uk0 + 1) & ~1, dLen = (dk1 - dk0 + 1) & ~1;                  // (whole 16-byte units)
+        const bool fits = ubCnt <= kK2StageBins && dbCnt <= kK2StageBins && uLen <= kK2StageHits && dLen <= kK2StageHits;
+        if (fits) {
+            if (threadIdx.x == 0) {
+                const uint32_t bytes = (uint32_t)(uLen + dLen) * (uint32_t)sizeof(float2);
+                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&sBar)), "r"(bytes) : "memory");
+                if (uLen > 0)
+                    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                                 ::"r"(smem_u32(sHitsU)), "l"(VU.hs + uk0), "r"((uint32_t)uLen * (uint32_t)sizeof(float2)), "r"(smem_u32(&sBar)) : "memory");
+                if (dLen > 0)
+                    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                                 ::"r"(smem_u32(sHitsD)), "l"(VD.hs + dk0), "r"((uint32_t)dLen * (uint32_t)sizeof(float2)), "r"(smem_u32(&sBar)) : "memory");
+            }
+            for (int b = threadIdx.x; b < ubCnt; b += kK2Threads) sBinsU[b] = VU.bs[ubBase + b];
+            for (int b = threadIdx.x; b < dbCnt; b += kK2Threads) sBinsD[b] = VD.bs[dbBase + b];
+            {   // wait for the bulk copies (phase 0 of the barrier)
+                uint32_t done = 0;
+                while (!done)
+                    asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\n selp.u32 %0, 1, 0, p;\n}"
+                                 : "=r"(done) : "r"(smem_u32(&sBar)) : "memory");
+            }
+            __syncthreads();
+            VU = K2Row{sHitsU, sBinsU, uk0, ubBase};
+            VD = K2Row{sHitsD, sBinsD, dk0, dbBase};
+        }
+    }
+
+    for (int i = i0 + threadIdx.x; i < i1; i += kK2Threads) {
         const float2 h = d.hits[R.hitOff + i];
         float cy[kK2Cap], cz[kK2Cap];
         int ck[kK2Cap];
         int nd = 0;
-        const WinRanges rD = win_ranges(Rd, d.binStart, h.x, h.y, wyD, wzD);
-        const WinRanges rU = win_ranges(Ru, d.binStart, h.x, h.y, wyU, wzU);
-        scan_ranges(rD, Rd, d.hits, d.binStart, [&](int k, float2 c) {
+        const WinRanges rD = k2_win_ranges(Rd, VD, h.x, h.y, wyD, wzD);
+        const WinRanges rU = k2_win_ranges(Ru, VU, h.x, h.y, wyU, wzU);
+        k2_scan(rD, Rd, VD, [&](int k, float2 c) {
             if (fabsf(c.x - h.x) <= wyD && fabsf(c.y - h.y) <= wzD) {
                 if (nd < kK2Cap) { cy[nd] = wd * c.x; cz[nd] = wd * c.y; ck[nd] = k; }
                 nd++;
@@ -316,7 +464,7 @@ __global__ void __launch_bounds__(kK2Threads, TPC_K2B) k2_neighbours(DevPtrs d, 
             if (better) { best = d2; bestU = ku; bestD = kd; }
         };
         if (nd > 0) {
-            scan_ranges(rU, Ru, d.hits, d.binStart, [&](int ku, float2 c) {
+            k2_scan(rU, Ru, VU, [&](int ku, float2 c) {
                 if (!(fabsf(c.x - h.x) <= wyU && fabsf(c.y - h.y) <= wzU)) return;
                 const float py = wu * c.x, pz = wu * c.y;
                 if (nd <= kK2Cap) {
@@ -325,7 +473,7 @@ __global__ void __launch_bounds__(kK2Threads, TPC_K2B) k2_neighbours(DevPtrs d, 
                         consider(ku, ck[j], ey * ey + ez * ez);
                     }
                 } else {
-                    for_window(Rd, d.hits, d.binStart, h.x, h.y, wyD, wzD, [&](int kd, float2 e) {
+                    k2_for_window(Rd, VD, h.x, h.y, wyD, wzD, [&](int kd, float2 e) {
                         if (!(fabsf(e.x - h.x) <= wyD && fabsf(e.y - h.y) <= wzD)) return;
                         const float ey = h.x - (py + wd * e.x), ez = h.y - (pz + wd * e.y);
                         consider(ku, kd, ey * ey + ez * ez);

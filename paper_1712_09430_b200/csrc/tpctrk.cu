@@ -66,6 +66,8 @@ struct tpc_tracker {
     uint32_t* hostCounters = nullptr;       // pinned
     uint32_t* hostRowStartBase = nullptr;   // pinned
     int maxBinsLaunch = 1;
+    int maxRowN = 0;                        // clusters in the fullest (sector,row) of the loaded event
+    bool k2Stage = false;                   // tpc_set_neighbour_staging
 
     // results (pinned)
     tpc_track* outTracks = nullptr; int64_t outTracksCap = 0;
@@ -214,7 +216,7 @@ int finalize_event(tpc_tracker* t) {
         t->tablesPending = false;                        // kernels behind it are not waited for)
     }
     int64_t gid = 0, hitOff = 0, binOff = 0;
-    int maxBins = 1;
+    int maxBins = 1, maxRow = 0;
     for (int i = 0; i < NR; i++) {
         RowGrid& G = t->hostGrid[i];
         RowMeta& M = t->hostMeta[i];
@@ -225,6 +227,7 @@ int finalize_event(tpc_tracker* t) {
         M.n = n; M.inOff = t->rowIn[i]; M.gidBase = (uint32_t)gid;
         M.maxBins = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)((double)n * (double)t->P.grid_bins_per_hit), kMaxBinsPerRow));
         maxBins = std::max(maxBins, M.maxBins);
+        maxRow = std::max(maxRow, n);
         gid += n;
         hitOff += (n + kRowPad - 1) / kRowPad * kRowPad;
         binOff += M.maxBins + 1;
@@ -241,6 +244,7 @@ int finalize_event(tpc_tracker* t) {
         if ((int64_t)t->hostSectorBase[s + 1] - (int64_t)t->hostSectorBase[s] > 0x00FFFFFF) return TPC_E_ARG;  // key field
     t->nClusters = gid;
     t->maxBinsLaunch = maxBins;
+    t->maxRowN = maxRow;
     if (gid > t->maxClusters || hitOff > t->L.hitCap || binOff > t->L.binCap) return TPC_E_NOMEM;
     CUDA_TRY(t, cudaMemcpyAsync(t->dev.grid, t->hostGrid, sizeof(RowGrid) * NR, cudaMemcpyHostToDevice, t->stream));
     CUDA_TRY(t, cudaMemcpyAsync((void*)t->dev.meta, t->hostMeta, sizeof(RowMeta) * NR, cudaMemcpyHostToDevice, t->stream));
@@ -468,6 +472,12 @@ int tpc_set_dependent_launch(tpc_tracker* t, int on) {
     return TPC_OK;
 }
 
+int tpc_set_neighbour_staging(tpc_tracker* t, int on) {
+    if (!t) return TPC_E_ARG;
+    t->k2Stage = on != 0;
+    return TPC_OK;
+}
+
 int tpc_set_output_prefetch(tpc_tracker* t, int on) {
     if (!t) return TPC_E_ARG;
     t->queueOutput = on != 0;
@@ -613,7 +623,17 @@ int tpc_track_sectors(tpc_tracker* t) {
 #endif
     const bool pdl = TPC_PDL && !timed && t->dependentLaunch;
     const int k5Blocks = t->k5Blocks, phW = kK5PhasedThreads / 32;
-    CUDA_TRY(t, launch_dep(pdl, k2_neighbours, NR, kK2Threads, 0, s, d, dp));
+    {   // K2: a block per chunk of kK2Chunk sorted hits of a (sector,row): grid.y = chunks of the fullest row
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3((unsigned)NR, (unsigned)std::max(1, (t->maxRowN + kK2Chunk - 1) / kK2Chunk));
+        cfg.blockDim = dim3(kK2Threads); cfg.stream = s;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
+        if (t->k2Stage) CUDA_TRY(t, cudaLaunchKernelEx(&cfg, k2_neighbours<true>, d, dp));
+        else CUDA_TRY(t, cudaLaunchKernelEx(&cfg, k2_neighbours<false>, d, dp));
+    }
     if (timed) CUDA_TRY(t, cudaEventRecord(t->ev[2], s));
     CUDA_TRY(t, launch_dep(pdl, k3_clean_start, NR, kK3Threads, 0, s, d, dp));
     if (timed) CUDA_TRY(t, cudaEventRecord(t->ev[3], s));

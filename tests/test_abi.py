@@ -33,7 +33,7 @@ def test_struct_layouts_match_header():
     p = binding.default_params()
     assert abs(p.err2_y - 0.01) < 1e-9 and p.min_hits == 10 and p.max_gap == 4 and p.seed_min_chain == 3
     assert abs(p.nf_tz - 1.5) < 1e-9 and abs(p.kf_ckk0 - 100.0) < 1e-9 and abs(p.road_max - 2.0) < 1e-9
-    assert abs(p.max_tracklets_per_cluster - 0.125) < 1e-9 and abs(p.grid_bins_per_hit - 3.0) < 1e-9
+    assert abs(p.max_tracklets_per_cluster - 0.1) < 1e-7 and abs(p.grid_bins_per_hit - 2.0) < 1e-9
 
 
 def test_create_validates_geometry():

@@ -622,3 +622,24 @@ def test_queued_download_and_fetching_the_rest():
     _, tracks, ids = run_gpu(big, tracker=trk)
     assert trk.get_stats()["n_output_refetches"] == 2          # nothing was queued: everything is "the rest"
     compare(big, trk, tracks, ids, ref_big)
+
+
+@pytest.mark.parametrize("cfg,seed,scale", [(3, 5, 1.0), (4, 0, 0.15)])
+def test_neighbour_staging_in_shared_memory_changes_no_result(cfg, seed, scale):
+    """tpc_set_neighbour_staging: K2 with the adjacent rows' pieces staged in shared memory by bulk copies (the
+    north_star's design) against the oracle, on a central event (a chunk = a whole row, the pieces = whole rows) and
+    on a thinned time frame (several chunks per row, pieces = bands in z; some chunks do not fit and read global)."""
+    torch = _cuda()
+    ev = datagen.config_event(cfg, seed=seed, scale=scale)
+    ref = oracle.run_event(ev)
+    trk = binding.Tracker(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz)
+    trk.set_stream(torch.cuda.current_stream().cuda_stream)
+    trk.allocate_workspace(ev.n_clusters)
+    trk.set_neighbour_staging(True)
+    _, tracks, ids = run_gpu(ev, tracker=trk)
+    out = compare(ev, trk, tracks, ids, ref)
+    assert out["link_mismatch_0"] == 0 and out["tracklet_mismatch"] == 0
+    links_staged = trk.debug_dump(binding.TPC_DUMP_LINKS).copy()
+    trk.set_neighbour_staging(False)
+    run_gpu(ev, tracker=trk)
+    assert np.array_equal(trk.debug_dump(binding.TPC_DUMP_LINKS), links_staged)
