@@ -635,7 +635,7 @@ int tpc_track_sectors(tpc_tracker* t) {
         else CUDA_TRY(t, cudaLaunchKernelEx(&cfg, k2_neighbours<false>, d, dp));
     }
     if (timed) CUDA_TRY(t, cudaEventRecord(t->ev[2], s));
-    CUDA_TRY(t, launch_dep(pdl, k3_clean_start, NR, kK3Threads, 0, s, d, dp));
+    CUDA_TRY(t, launch_dep(pdl, k3_clean_start, NR, kK3Threads, 0, s, d, dp, t->nClusters > (int64_t)1000 * NR ? 1 : 0));
     if (timed) CUDA_TRY(t, cudaEventRecord(t->ev[3], s));
     // K5: one persistent block per SM; the phased and the free-running instantiation decide on the device (from the
     // number of start hits) which of them does the event, the other returns at once
