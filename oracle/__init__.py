@@ -26,6 +26,8 @@ class Params(ctypes.Structure):
         ("kf_smax", ctypes.c_double), ("road_nsig", ctypes.c_double), ("road_max", ctypes.c_double),
         ("max_gap", ctypes.c_int32), ("min_hits", ctypes.c_int32), ("seed_min_chain", ctypes.c_int32),
         ("pad", ctypes.c_int32),
+        ("merge_chi2", ctypes.c_double), ("merge_max_row_gap", ctypes.c_int32), ("pad2", ctypes.c_int32),
+        ("sector_dphi", ctypes.c_double),
     ]
 
 
@@ -82,6 +84,14 @@ def lib():
         L.oracle_propagate.restype = i32
         L.oracle_propagate.argtypes = [i32, vp, vp, vp, dbl, dbl, dbl, vp]
         L.oracle_update.argtypes = [i32, vp, vp, vp, i32, dbl, dbl]
+        L.oracle_merge.argtypes = [vp]
+        L.oracle_n_merged.restype = i64
+        L.oracle_n_merged.argtypes = [vp]
+        L.oracle_get_merge.argtypes = [vp] + [vp] * 6
+        L.oracle_rotate.restype = i32
+        L.oracle_rotate.argtypes = [i32, vp, vp, vp, dbl, dbl, dbl]
+        L.oracle_chi2_5.restype = dbl
+        L.oracle_chi2_5.argtypes = [i32, vp, vp]
         assert L.oracle_sizeof_tracklet() == TRACKLET_DTYPE.itemsize, (L.oracle_sizeof_tracklet(), TRACKLET_DTYPE.itemsize)
         assert L.oracle_sizeof_track() == TRACK_DTYPE.itemsize, (L.oracle_sizeof_track(), TRACK_DTYPE.itemsize)
         _lib = L
@@ -129,6 +139,18 @@ class Oracle:
         L.oracle_run(self._h, rc.ctypes.data, y.ctypes.data, z.ctypes.data, 1 if brute_force else 0)
         return self.fetch() if fetch else None
 
+    def merge(self, res: "Result") -> "Result":
+        """Phase II track merging (S7) on the tracks of the last run; adds the merge_* fields to ``res``."""
+        L, h = lib(), self._h
+        L.oracle_merge(h)
+        n, m = res.tracks.size, int(L.oracle_n_merged(h))
+        res.merge_next, res.merge_prev = np.empty(n, np.int32), np.empty(n, np.int32)
+        res.merge_chi2, res.merge_tie = np.empty(n, np.float64), np.empty(n, np.uint8)
+        res.merged_offset, res.merged_segs = np.empty(m + 1, np.int32), np.empty(n, np.int32)
+        L.oracle_get_merge(h, res.merge_next.ctypes.data, res.merge_prev.ctypes.data, res.merge_chi2.ctypes.data,
+                           res.merge_tie.ctypes.data, res.merged_offset.ctypes.data, res.merged_segs.ctypes.data)
+        return res
+
     def stage_seconds(self):
         s = np.zeros(6)
         lib().oracle_get_stage_seconds(self._h, s.ctypes.data)
@@ -167,6 +189,26 @@ def run_event(ev, params: Params | None = None, precision="float", brute_force=F
     """Convenience: run the oracle on a datagen.Event-like object (duck-typed, no import of datagen)."""
     o = Oracle(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz, params, precision)
     return o.run(ev.row_counts, ev.y, ev.z, brute_force)
+
+
+def run_event_merged(ev, params: Params | None = None, precision="float") -> Result:
+    """Phase I + Phase II merging on a datagen.Event-like object."""
+    o = Oracle(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz, params, precision)
+    return o.merge(o.run(ev.row_counts, ev.y, ev.z))
+
+
+def rotate(x, p, c, beta, cb, smax=0.95, precision="double"):
+    """Rotate a state into the frame turned by +beta about z; returns (ok, x', p'[5], c'[15])."""
+    xa = np.array([x], dtype=np.float64)
+    pa, ca = np.array(p, dtype=np.float64).copy(), np.array(c, dtype=np.float64).copy()
+    ok = lib().oracle_rotate(1 if precision == "double" else 0, xa.ctypes.data, pa.ctypes.data, ca.ctypes.data,
+                             float(beta), float(cb), float(smax))
+    return bool(ok), float(xa[0]), pa, ca
+
+
+def chi2_5(d, s15, precision="double"):
+    da, sa = np.ascontiguousarray(d, dtype=np.float64), np.ascontiguousarray(s15, dtype=np.float64)
+    return float(lib().oracle_chi2_5(1 if precision == "double" else 0, da.ctypes.data, sa.ctypes.data))
 
 
 def propagate(x, p, c, x2, cb, smax=0.95, precision="double"):

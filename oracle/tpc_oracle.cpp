@@ -45,6 +45,10 @@ struct ParamsD {                 /* DESIGN.md "Constants" */
     double kf_smax;              /* |sin(phi)| limit of the propagation */
     double road_nsig, road_max;  /* search road */
     int32_t max_gap, min_hits, seed_min_chain, pad;
+    double merge_chi2;           /* S7: max chi2 (5 dof) of two matching track segments */
+    int32_t merge_max_row_gap;   /* S7: max pad rows between the end of the inner and the start of the outer segment */
+    int32_t pad2;
+    double sector_dphi;          /* S7: angle between neighbouring sector frames [rad] */
 };
 
 /* ------------------------------------------------------------------ track model (S5) */
@@ -141,6 +145,70 @@ template <class T> void update_hit(State<T> &st, T ym, T zm, T e2y, T e2z) {
     update1(st, 0, ym, e2y);
     update1(st, 1, zm, e2z);
     st.nfit++;
+}
+
+/* ------------------------------------------------------------------ Phase II: track merging (S7) */
+/* Express the state in a frame rotated by +beta about z (x' = x cos b + y sin b, y' = -x sin b + y cos b), at the
+ * plane x' = const through the state's own point.  cb, sb = cos/sin(beta) in working precision.  The track is assumed
+ * to move towards +x in both frames (cos phi > 0); returns false (state untouched) if it does not in the new one or if
+ * |sin phi'| >= smax.  Covariance: C' = J C J^T with the Jacobian of "rotate, then slide along the track back to
+ * the plane" (S7): dy'/dy = c/c', dz'/dy = -t sb/c', ds'/dy = -k CB sb, ds'/ds = c'/c. */
+template <class T> bool rotate(State<T> &st, T cb, T sb, T CB, T smax) {
+    const T y = st.p[0], s = st.p[2], t = st.p[3], k = st.p[4];
+    const T c = std::sqrt(T(1) - s * s);
+    const T s2 = s * cb - c * sb;
+    const T c2 = c * cb + s * sb;
+    if (!(c2 > T(0)) || !(std::fabs(s2) < smax) || !(std::fabs(s) < smax)) return false;
+    T J[5][5];
+    for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) J[i][j] = (i == j) ? T(1) : T(0);
+    J[0][0] = c / c2;
+    J[1][0] = -(t * sb) / c2;
+    J[2][0] = -((k * CB) * sb);
+    J[2][2] = c2 / c;
+    T A[5][5], C2[5][5];
+    for (int i = 0; i < 5; i++)
+        for (int j = 0; j < 5; j++) {
+            T acc = T(0);
+            for (int m = 0; m < 5; m++) acc = acc + J[i][m] * st.C[m][j];
+            A[i][j] = acc;
+        }
+    for (int i = 0; i < 5; i++)
+        for (int j = 0; j <= i; j++) {
+            T acc = T(0);
+            for (int m = 0; m < 5; m++) acc = acc + A[i][m] * J[j][m];
+            C2[i][j] = acc; C2[j][i] = acc;
+        }
+    const T xn = st.x * cb + y * sb;
+    st.p[0] = y * cb - st.x * sb;
+    st.x = xn;
+    st.p[2] = s2;
+    std::memcpy(st.C, C2, sizeof(C2));
+    return true;
+}
+
+/* chi2 = d^T S^-1 d for symmetric positive definite S (5x5), by LDL^T without pivoting; returns a huge value if a
+ * pivot is not positive (then the two covariances carry no information and nothing is merged). */
+template <class T> T chi2_5(const T d[5], const T S[5][5]) {
+    T L[5][5], D[5];
+    for (int j = 0; j < 5; j++) {
+        T dj = S[j][j];
+        for (int m = 0; m < j; m++) dj = dj - (L[j][m] * L[j][m]) * D[m];
+        if (!(dj > T(0))) return T(1e30);
+        D[j] = dj;
+        for (int i = j + 1; i < 5; i++) {
+            T v = S[i][j];
+            for (int m = 0; m < j; m++) v = v - (L[i][m] * L[j][m]) * D[m];
+            L[i][j] = v / dj;
+        }
+    }
+    T w[5], chi = T(0);
+    for (int i = 0; i < 5; i++) {               /* forward substitution L w = d, then sum w^2 / D */
+        T v = d[i];
+        for (int m = 0; m < i; m++) v = v - L[i][m] * w[m];
+        w[i] = v;
+        chi = chi + (v * v) / D[i];
+    }
+    return chi;
 }
 
 /* ------------------------------------------------------------------ the tracker */
@@ -465,6 +533,75 @@ template <class T> struct Tracker {
         }
     }
 
+    /* ---------------------------------------------------------------- S7 track merging (Phase II) */
+    /* Per Phase-I track i (index into tracks): the segment that continues it outward / inward, -1 none. */
+    std::vector<int32_t> mergeNext, mergePrev;
+    std::vector<double> mergeChi2;          /* chi2 of the link i -> mergeNext[i] */
+    std::vector<uint8_t> mergeTie;          /* the decision for track i was within 1e-6 relative of another one */
+    std::vector<int32_t> mergedOffset, mergedSegs;   /* merged tracks: segments of merged track m = mergedSegs[off[m]..off[m+1]) */
+
+    /* chi2 between segment a (inner) and segment b (outer): a's state is brought into b's sector frame and to b's
+     * reference x (rotate, then propagate), then compared with b's state using the sum of the covariances.  < 0: no
+     * match possible (different side, not neighbouring sectors, wrong order in rows, propagation fails). */
+    T pairChi2(const TrackOut &a, const TrackOut &b) const {
+        const int perSide = nSec >= 36 ? 18 : nSec;          /* sectors per TPC half (fewer in small test geometries) */
+        if (a.sector / perSide != b.sector / perSide) return T(-1);
+        const int sa = a.sector % perSide, sb_ = b.sector % perSide;
+        int dsec = sb_ - sa;                                  /* -1, 0, +1 modulo the ring */
+        if (dsec > perSide / 2) dsec -= perSide;
+        if (dsec < -perSide / 2) dsec += perSide;
+        if (dsec < -1 || dsec > 1) return T(-1);
+        if (!(b.first_row > a.last_row) || b.first_row - a.last_row > pd.merge_max_row_gap) return T(-1);
+        State<T> st;
+        st.x = T(a.x); st.chi2 = T(0); st.nfit = 0;
+        for (int i = 0; i < 5; i++) st.p[i] = T(a.p[i]);
+        for (int i = 0, k = 0; i < 5; i++) for (int j = 0; j <= i; j++) { st.C[i][j] = st.C[j][i] = T(a.c[k++]); }
+        if (dsec != 0) {
+            const double beta = double(dsec) * pd.sector_dphi;       /* b's frame is a's rotated by +beta */
+            if (!rotate(st, T(std::cos(beta)), T(std::sin(beta)), CB, smax)) return T(-1);
+        }
+        if (!propagate(st, T(b.x), CB, smax)) return T(-1);
+        T d[5], S[5][5];
+        for (int i = 0; i < 5; i++) d[i] = st.p[i] - T(b.p[i]);
+        for (int i = 0, k = 0; i < 5; i++) for (int j = 0; j <= i; j++) { const T v = st.C[i][j] + T(b.c[k++]); S[i][j] = v; S[j][i] = v; }
+        return chi2_5(d, S);
+    }
+
+    void mergeTracks() {
+        const int n = int(tracks.size());
+        mergeNext.assign(n, -1); mergePrev.assign(n, -1); mergeChi2.assign(n, 0.0); mergeTie.assign(n, 0);
+        std::vector<T> bestOut(n, T(0)), bestIn(n, T(0));
+        std::vector<int32_t> out(n, -1), in(n, -1);
+        const T cut = T(pd.merge_chi2);
+        /* canonical key of a track = id of its first cluster */
+        auto key = [&](int i) { return clusterIds[tracks[i].cluster_offset]; };
+        for (int a = 0; a < n; a++)
+            for (int b = 0; b < n; b++) {
+                if (a == b) continue;
+                const T c = pairChi2(tracks[a], tracks[b]);
+                if (c < T(0)) continue;
+                if (nearRel(c, cut)) { mergeTie[a] = 1; mergeTie[b] = 1; }
+                if (!(c <= cut)) continue;
+                /* best outer partner of a, best inner partner of b: smaller chi2, then smaller key */
+                if (out[a] >= 0 && nearRel(c, bestOut[a])) mergeTie[a] = 1;
+                if (out[a] < 0 || c < bestOut[a] || (c == bestOut[a] && key(b) < key(out[a]))) { out[a] = b; bestOut[a] = c; }
+                if (in[b] >= 0 && nearRel(c, bestIn[b])) mergeTie[b] = 1;
+                if (in[b] < 0 || c < bestIn[b] || (c == bestIn[b] && key(a) < key(in[b]))) { in[b] = a; bestIn[b] = c; }
+            }
+        /* a link survives if it is mutual (as in the neighbours cleaner, S3) */
+        for (int a = 0; a < n; a++)
+            if (out[a] >= 0 && in[out[a]] == a) { mergeNext[a] = out[a]; mergePrev[out[a]] = a; mergeChi2[a] = double(bestOut[a]); }
+        /* merged tracks: chains from the segments without an inner partner, in ascending key of that segment */
+        std::vector<int> heads;
+        for (int i = 0; i < n; i++) if (mergePrev[i] < 0) heads.push_back(i);
+        std::sort(heads.begin(), heads.end(), [&](int x, int y) { return key(x) < key(y); });
+        mergedOffset.assign(1, 0); mergedSegs.clear();
+        for (int h : heads) {
+            for (int i = h; i >= 0; i = mergeNext[i]) mergedSegs.push_back(i);
+            mergedOffset.push_back(int32_t(mergedSegs.size()));
+        }
+    }
+
     void run(const int32_t *rowCounts, const float *yin, const float *zin, int bruteForce) {
         using clk = std::chrono::steady_clock;
         brute = bruteForce != 0;
@@ -540,6 +677,8 @@ void oracle_default_params(ParamsD *p) {
     p->kf_css0 = 1.0; p->kf_ctt0 = 10.0; p->kf_ckk0 = 100.0; p->kf_smax = 0.95;
     p->road_nsig = 4.0; p->road_max = 2.0;
     p->max_gap = 4; p->min_hits = 10; p->seed_min_chain = 3; p->pad = 0;
+    p->merge_chi2 = 50.0; p->merge_max_row_gap = 40; p->pad2 = 0;
+    p->sector_dphi = 20.0 * 3.14159265358979323846 / 180.0;
 }
 
 void *oracle_create(int n_sectors, int n_rows, const float *row_x, double bz, const ParamsD *p, int use_double) {
@@ -607,6 +746,46 @@ void oracle_get_tracks(void *hv, void *dst, int32_t *cluster_ids) {
 void oracle_get_stage_seconds(void *hv, double *dst) {
     Handle *h = (Handle *)hv;
     std::memcpy(dst, h->useDouble ? h->d->stageSec : h->f->stageSec, 6 * sizeof(double));
+}
+
+/* ---- Phase II (S7): run after oracle_run; results indexed like the tracks of oracle_get_tracks ---- */
+void oracle_merge(void *hv) { Handle *h = (Handle *)hv; if (h->useDouble) h->d->mergeTracks(); else h->f->mergeTracks(); }
+int64_t oracle_n_merged(void *hv) { Handle *h = (Handle *)hv; return (int64_t)DISPATCH(h, mergedOffset.size()) - 1; }
+void oracle_get_merge(void *hv, int32_t *next, int32_t *prev, double *chi2, uint8_t *tie, int32_t *merged_offset, int32_t *merged_segs) {
+    Handle *h = (Handle *)hv;
+    auto cp = [&](auto &t) {
+        const size_t n = t.mergeNext.size();
+        std::memcpy(next, t.mergeNext.data(), n * 4); std::memcpy(prev, t.mergePrev.data(), n * 4);
+        std::memcpy(chi2, t.mergeChi2.data(), n * 8); std::memcpy(tie, t.mergeTie.data(), n);
+        std::memcpy(merged_offset, t.mergedOffset.data(), t.mergedOffset.size() * 4);
+        std::memcpy(merged_segs, t.mergedSegs.data(), t.mergedSegs.size() * 4);
+    };
+    if (h->useDouble) cp(*h->d); else cp(*h->f);
+}
+/* primitives for the pins: rotate a state (x[1], p[5], c[15]) by beta; chi2 of d with covariance S (15) */
+int oracle_rotate(int use_double, double *x, double *p, double *c, double beta, double CB, double smax) {
+    auto run = [&](auto tag) {
+        using T = decltype(tag);
+        State<T> st; st.x = T(*x); st.chi2 = T(0); st.nfit = 0;
+        for (int i = 0; i < 5; i++) st.p[i] = T(p[i]);
+        for (int i = 0, k = 0; i < 5; i++) for (int j = 0; j <= i; j++) { st.C[i][j] = st.C[j][i] = T(c[k++]); }
+        if (!rotate(st, T(std::cos(beta)), T(std::sin(beta)), T(CB), T(smax))) return 0;
+        *x = double(st.x);
+        for (int i = 0; i < 5; i++) p[i] = double(st.p[i]);
+        for (int i = 0, k = 0; i < 5; i++) for (int j = 0; j <= i; j++) c[k++] = double(st.C[i][j]);
+        return 1;
+    };
+    return use_double ? run(double(0)) : run(float(0));
+}
+double oracle_chi2_5(int use_double, const double *d, const double *s15) {
+    auto run = [&](auto tag) {
+        using T = decltype(tag);
+        T dd[5], S[5][5];
+        for (int i = 0; i < 5; i++) dd[i] = T(d[i]);
+        for (int i = 0, k = 0; i < 5; i++) for (int j = 0; j <= i; j++) { S[i][j] = S[j][i] = T(s15[k++]); }
+        return double(chi2_5(dd, S));
+    };
+    return use_double ? run(double(0)) : run(float(0));
 }
 
 int oracle_propagate(int use_double, double *x, double *p, double *c, double x2, double CB, double smax, double *J) {
