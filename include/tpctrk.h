@@ -58,13 +58,17 @@ typedef struct tpc_params {
     float max_tracklets_per_cluster;/* capacity estimate for tracklets                      0.1 */
     float grid_bins_per_hit;        /* resolution of the per-row y/z grid (accelerator only: no result
                                        depends on it), bins per cluster of the row, 0.25..64                2 */
+    float merge_chi2;               /* Phase II merging: max chi2 (5 parameters) of two matching segments  50 */
+    int32_t merge_max_row_gap;      /* ... max pad rows between the end of the inner segment and the
+                                       start of the outer one                                              40 */
 } tpc_params;
 
 typedef struct tpc_geometry {
     int32_t n_sectors;        /* 36: s<18 side A (z>0), s>=18 side C (z<0); any value >= 1 works */
     int32_t n_rows;           /* 159 pad rows; 3 <= n_rows <= 255 */
     const float* row_x;       /* host pointer, n_rows ascending pad-row x [cm]; copied at create */
-    float sector_dphi;        /* informational: 20 deg in rad; all tracking is sector-local */
+    float sector_dphi;        /* angle between the frames of neighbouring sectors [rad] (20 deg); Phase I is sector-local
+                                 and does not use it, tpc_merge_tracks rotates states by it */
     float z_max;              /* informational: drift length [cm] */
     const tpc_params* params; /* host pointer or NULL = defaults */
 } tpc_geometry;
@@ -87,6 +91,9 @@ typedef struct tpc_stats {
     int64_t workspace_bytes_used, max_clusters, max_tracklets;
     int64_t n_output_refetches; /* calls of tpc_get_tracks (since create) that had to fetch a remainder because the
                                  download queued by tpc_track_sectors was estimated too small */
+    float merge_us;           /* device time of the last tpc_merge_tracks (K7), valid after tpc_get_merged */
+    int32_t n_merged_tracks, n_merge_links;   /* after tpc_get_merged */
+    int32_t pad_;
     float kernel_us[8];       /* K1 sort+grid, K2 neighbours, K3/K4 clean+start, K5 construct, K6a weights,
                                  K6b select+compact, [6] = K1..K6 total, [7] = 1.0 if the K6a weights pass of this
                                  event ran inside the K5 launch (about one tracklet per GPU thread or fewer: [3]
@@ -192,6 +199,31 @@ int tpc_get_tracks(tpc_tracker* t, const tpc_track** tracks, int32_t* n_tracks,
 /* Wait for the last tpc_track_sectors and its queued download; counters + per-kernel device times only. */
 int tpc_sync(tpc_tracker* t);
 int tpc_get_stats(tpc_tracker* t, tpc_stats* out);
+
+/* ---- Phase II, first step: track merging (Table 1 "Matching Covariance"; reading S7 of DESIGN.md) ----
+ * A merged track = a chain of Phase-I tracks ("segments") of one TPC side, each continued outward by the segment in
+ * the same or a neighbouring sector that starts within merge_max_row_gap pad rows above its end and whose state is
+ * nearest in chi2 (<= merge_chi2) after the inner state has been rotated into the outer segment's sector frame and
+ * propagated to its x; a link is kept only if it is the best one from both ends.  Sectors s and s+1 (mod 18 within
+ * a side; n_sectors < 36: one ring of all sectors) are neighbours, sector s+1's frame is sector s's turned by
+ * +sector_dphi.  Parameters are those of the segments (no refit: PAPER.md:46 is a later step). */
+typedef struct tpc_merged_track {
+    int32_t n_segments;       /* 1 = a Phase-I track nothing was merged with */
+    int32_t n_clusters;       /* sum over the segments */
+    int32_t segment_offset;   /* into segments[]: track indices (as in tpc_get_tracks), innermost segment first */
+    int32_t first_track;      /* = segments[segment_offset] */
+} tpc_merged_track;
+
+/* Run the merging kernels (K7) on the tracks of the last tpc_track_sectors, on the stream.  Asynchronous.
+ * TPC_E_STATE before tpc_track_sectors. */
+int tpc_merge_tracks(tpc_tracker* t);
+
+/* Synchronise and download.  next[i] / prev[i]: index of the segment that continues track i outward / inward, -1
+ * none; chi2[i]: chi2 of the link i -> next[i] (0 without link); n_tracks entries each, indexed like the arrays of
+ * tpc_get_tracks of the same event.  merged[n_merged] in unspecified order, segments[n_tracks].  Library-owned
+ * pinned memory, valid until the next merge/track/reset/destroy.  Any output pointer may be NULL. */
+int tpc_get_merged(tpc_tracker* t, const int32_t** next, const int32_t** prev, const float** chi2, int32_t* n_tracks,
+                   const tpc_merged_track** merged, int32_t* n_merged, const int32_t** segments);
 
 /* Stage parity hooks (tests): copy one stage's buffers, converted to canonical (load-index) form, to host_dst.
  * Synchronous; allocates temporary device memory.  bytes must equal tpc_debug_dump_bytes(t, stage). */

@@ -23,6 +23,7 @@ class tpc_params(ctypes.Structure):
         ("road_nsig", ctypes.c_float), ("road_max", ctypes.c_float), ("max_gap", ctypes.c_int32),
         ("min_hits", ctypes.c_int32), ("seed_min_chain", ctypes.c_int32),
         ("max_tracklets_per_cluster", ctypes.c_float), ("grid_bins_per_hit", ctypes.c_float),
+        ("merge_chi2", ctypes.c_float), ("merge_max_row_gap", ctypes.c_int32),
     ]
 
 
@@ -39,6 +40,7 @@ class tpc_stats(ctypes.Structure):
         ("n_tracklets", ctypes.c_int64), ("n_tracklet_hits", ctypes.c_int64), ("n_tracks", ctypes.c_int64),
         ("n_track_clusters", ctypes.c_int64), ("workspace_bytes_used", ctypes.c_int64),
         ("max_clusters", ctypes.c_int64), ("max_tracklets", ctypes.c_int64), ("n_output_refetches", ctypes.c_int64),
+        ("merge_us", ctypes.c_float), ("n_merged_tracks", ctypes.c_int32), ("n_merge_links", ctypes.c_int32), ("pad_", ctypes.c_int32),
         ("kernel_us", ctypes.c_float * 8),
     ]
 
@@ -51,6 +53,7 @@ TRACKLET_DTYPE = np.dtype([
     ("start_gid", np.uint32), ("sector", np.int32), ("start_row", np.int32), ("n_hits", np.int32),
     ("first_row", np.int32), ("last_row", np.int32), ("n_fit", np.int32), ("x", np.float32),
     ("p", np.float32, 5), ("c", np.float32, 15), ("chi2", np.float32)])
+MERGED_DTYPE = np.dtype([("n_segments", np.int32), ("n_clusters", np.int32), ("segment_offset", np.int32), ("first_track", np.int32)])
 assert TRACK_DTYPE.itemsize == 112 and TRACKLET_DTYPE.itemsize == 116
 
 TPC_OK, TPC_E_ARG, TPC_E_STATE, TPC_E_NOMEM, TPC_E_OVERFLOW, TPC_E_CUDA = 0, -1, -2, -3, -4, -5
@@ -93,6 +96,9 @@ def lib():
         L.tpc_track_sectors.argtypes = [vp]
         L.tpc_get_tracks.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(i32), ctypes.POINTER(vp), ctypes.POINTER(i64)]
         L.tpc_sync.argtypes = [vp]
+        L.tpc_merge_tracks.argtypes = [vp]
+        L.tpc_get_merged.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(i32),
+                                     ctypes.POINTER(vp), ctypes.POINTER(i32), ctypes.POINTER(vp)]
         L.tpc_get_stats.argtypes = [vp, ctypes.POINTER(tpc_stats)]
         L.tpc_debug_dump_bytes.argtypes = [vp, i32]
         L.tpc_debug_dump_bytes.restype = ctypes.c_size_t
@@ -235,10 +241,30 @@ class Tracker:
             tracks, ids = tracks.copy(), ids.copy()
         return (tracks, ids, rc) if allow_overflow else (tracks, ids)
 
+    def merge_tracks(self):
+        return self._check(self._L.tpc_merge_tracks(self._h), "tpc_merge_tracks")
+
+    def get_merged(self):
+        """-> dict(next, prev, chi2 per track; merged records; segments)."""
+        nx, pv, ch, mg, sg = (ctypes.c_void_p() for _ in range(5))
+        nt, nm = ctypes.c_int32(), ctypes.c_int32()
+        self._check(self._L.tpc_get_merged(self._h, ctypes.byref(nx), ctypes.byref(pv), ctypes.byref(ch), ctypes.byref(nt),
+                                           ctypes.byref(mg), ctypes.byref(nm), ctypes.byref(sg)), "tpc_get_merged")
+
+        def arr(p, n, dt):
+            if not n:
+                return np.zeros(0, dtype=dt)
+            buf = (ctypes.c_char * (n * np.dtype(dt).itemsize)).from_address(p.value)
+            return np.frombuffer(buf, dtype=dt).copy()
+        n, m = nt.value, nm.value
+        return {"next": arr(nx, n, np.int32), "prev": arr(pv, n, np.int32), "chi2": arr(ch, n, np.float32),
+                "merged": arr(mg, m, MERGED_DTYPE), "segments": arr(sg, n, np.int32)}
+
     def get_stats(self) -> dict:
         s = tpc_stats()
         self._check(self._L.tpc_get_stats(self._h, ctypes.byref(s)), "tpc_get_stats")
-        d = {k: int(getattr(s, k)) for k, _ in tpc_stats._fields_ if k != "kernel_us"}
+        d = {k: int(getattr(s, k)) for k, _ in tpc_stats._fields_ if k not in ("kernel_us", "merge_us")}
+        d["merge_us"] = float(s.merge_us)
         d["kernel_us"] = dict(zip(KERNEL_NAMES, [float(v) for v in s.kernel_us[:6]]))
         d["total_us"] = float(s.kernel_us[6])
         d["k6a_fused"] = bool(s.kernel_us[7] > 0.5)

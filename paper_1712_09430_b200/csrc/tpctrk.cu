@@ -13,6 +13,7 @@
 #include "device_types.cuh"
 #include "kernels_ca.cuh"
 #include "kernels_kf.cuh"
+#include "kernels_merge.cuh"
 
 using namespace tpc;
 
@@ -23,7 +24,8 @@ inline size_t align_up(size_t v, size_t a = kAlign) { return (v + a - 1) / a * a
 
 struct Layout {   // byte offsets into the workspace
     size_t inY, inZ, grid, meta, rowX, hits, orig, binStart, buckets, linkUp, linkDn, linkUpC, linkDnC, weight, starts, startsRaw, rowHist, rowStartBase, recs, rowHit,
-        tracks, clusterIds, counters, sectorGidBase, total;
+        tracks, clusterIds, counters, sectorGidBase,
+        mKey, mBinStart, mBinCursor, mOrder, mBestIn, mOut, mOutChi2, mNext, mPrev, mChi2, mMerged, mSegments, mCount, total;
     int64_t hitCap, binCap, maxTracklets;
 };
 
@@ -59,7 +61,15 @@ struct tpc_tracker {
     int64_t estTracks = 0, estIds = 0;      // size of the download that is queued before the counts are known
     int64_t queuedTracks = 0, queuedIds = 0;   // ... what the last tpc_track_sectors queued
     bool queueOutput = true;                // tpc_set_output_prefetch
-    int64_t nRefetch = 0;                   // how often the estimate was short (tpc_stats)
+    int64_t nRefetch = 0;
+    // Phase II merging
+    float sectorDphi = 0.f;
+    MergePtrs mp{};
+    bool merged = false, mergeFetched = false;
+    cudaEvent_t evM0 = nullptr, evM1 = nullptr;
+    int32_t* outNext = nullptr; int32_t* outPrev = nullptr; float* outMChi2 = nullptr; tpc_merged_track* outMerged = nullptr;
+    int32_t* outSegments = nullptr; uint32_t* outMCount = nullptr; int64_t outMergeCap = 0;
+    float mergeUs = 0.f; int32_t nMerged = 0, nMergeLinks = 0;                   // how often the estimate was short (tpc_stats)
     RowGrid* hostGrid = nullptr;            // pinned
     RowMeta* hostMeta = nullptr;            // pinned
     uint32_t* hostSectorBase = nullptr;     // pinned
@@ -120,6 +130,11 @@ Layout make_layout(const tpc_tracker* t, int64_t maxClusters) {
     L.clusterIds = take(sizeof(uint32_t) * (maxClusters + 16));
     L.counters = take(sizeof(uint32_t) * (kNCounters + kMaxPending));
     L.sectorGidBase = take(sizeof(uint32_t) * (t->nSec + 1));
+    // K7 (Phase II merging): per-track words, sized like the track output
+    const int64_t TC = L.maxTracklets;
+    L.mKey = take(4 * TC); L.mOrder = take(4 * TC); L.mBestIn = take(8 * TC); L.mOut = take(4 * TC); L.mOutChi2 = take(4 * TC);
+    L.mNext = take(4 * TC); L.mPrev = take(4 * TC); L.mChi2 = take(4 * TC); L.mMerged = take(sizeof(tpc_merged_track) * TC);
+    L.mSegments = take(4 * TC); L.mBinStart = take(4 * (NR + 4)); L.mBinCursor = take(4 * (NR + 4)); L.mCount = take(16);
     L.total = o;
     return L;
 }
@@ -152,6 +167,13 @@ void bind_pointers(tpc_tracker* t) {
     d.counters = (uint32_t*)(w + L.counters); d.sectorGidBase = (uint32_t*)(w + L.sectorGidBase);
     d.nRowsTotal = t->nRowsTotal; d.maxTracklets = (int32_t)std::min<int64_t>(L.maxTracklets, 0x7fffffff);
     d.rhStride = t->rhStride;
+    MergePtrs& m = t->mp;
+    m.tracks = d.tracks; m.clusterIds = d.clusterIds; m.counters = d.counters;
+    m.key = (uint32_t*)(w + L.mKey); m.binStart = (uint32_t*)(w + L.mBinStart); m.binCursor = (uint32_t*)(w + L.mBinCursor);
+    m.order = (uint32_t*)(w + L.mOrder); m.bestIn = (unsigned long long*)(w + L.mBestIn); m.out = (int32_t*)(w + L.mOut);
+    m.outChi2 = (float*)(w + L.mOutChi2); m.next = (int32_t*)(w + L.mNext); m.prev = (int32_t*)(w + L.mPrev);
+    m.chi2 = (float*)(w + L.mChi2); m.merged = (tpc_merged_track*)(w + L.mMerged); m.segments = (int32_t*)(w + L.mSegments);
+    m.mcount = (uint32_t*)(w + L.mCount); m.nBins = t->nRowsTotal;
 }
 
 // Page-locked host memory (cudaMallocHost / cudaHostRegister, e.g. a pinned torch tensor): the DMA engine can read it
@@ -405,6 +427,7 @@ void tpc_default_params(tpc_params* p) {
     p->kf_css0 = 1.0f; p->kf_ctt0 = 10.0f; p->kf_ckk0 = 100.0f; p->kf_smax = 0.95f;
     p->road_nsig = 4.0f; p->road_max = 2.0f;
     p->max_gap = 4; p->min_hits = 10; p->seed_min_chain = 3;
+    p->merge_chi2 = 50.0f; p->merge_max_row_gap = 40;
     p->max_tracklets_per_cluster = 0.1f;
     p->grid_bins_per_hit = 2.0f;
 }
@@ -431,9 +454,10 @@ int tpc_tracker_create(const tpc_geometry* g, float bz_tesla, tpc_tracker** out)
                         pos(P.road_nsig) && pos(P.road_max) && P.kf_smax > 0.f && P.kf_smax < 1.f &&
                         nonneg(P.nf_ty) && nonneg(P.nf_tz) && nonneg(P.nf_c) && nonneg(P.nf_d2max) &&
                         P.seed_min_chain >= 2 && P.min_hits >= 1 && P.max_gap >= 0 && pos(P.max_tracklets_per_cluster) &&
-                        P.grid_bins_per_hit >= 0.25f && P.grid_bins_per_hit <= 64.f && bz_tesla == bz_tesla && std::abs(bz_tesla) < 1e3f;
+                        P.grid_bins_per_hit >= 0.25f && P.grid_bins_per_hit <= 64.f && nonneg(P.merge_chi2) && P.merge_max_row_gap >= 0 && bz_tesla == bz_tesla && std::abs(bz_tesla) < 1e3f;
         if (!ok) { delete t; return TPC_E_ARG; }
     }
+    t->sectorDphi = g->sector_dphi;
     t->bz = bz_tesla;
     t->CB = (float)(-0.299792458e-2 * (double)bz_tesla);   // kappa = (q/pT) * CB, constant field
     t->rowN.assign(t->nRowsTotal, 0); t->rowIn.assign(t->nRowsTotal, 0); t->rowCap.assign(t->nRowsTotal, 0);
@@ -457,6 +481,10 @@ void tpc_tracker_destroy(tpc_tracker* t) {
     if (t->evUpload) cudaEventDestroy(t->evUpload);
     if (t->evTables) cudaEventDestroy(t->evTables);
     if (t->evDone) cudaEventDestroy(t->evDone);
+    if (t->evM0) cudaEventDestroy(t->evM0);
+    if (t->evM1) cudaEventDestroy(t->evM1);
+    for (void* q : {(void*)t->outNext, (void*)t->outPrev, (void*)t->outMChi2, (void*)t->outMerged, (void*)t->outSegments, (void*)t->outMCount})
+        if (q) cudaFreeHost(q);
     delete t;
 }
 
@@ -658,7 +686,77 @@ int tpc_track_sectors(tpc_tracker* t) {
     // tpc_get_tracks waits once and normally copies nothing.
     rc = queue_download(t);
     if (rc != TPC_OK) return rc;
-    t->tracked = true; t->fetched = false;
+    t->tracked = true; t->fetched = false; t->merged = false; t->mergeFetched = false;
+    return TPC_OK;
+}
+
+int tpc_merge_tracks(tpc_tracker* t) {
+    if (!t) return TPC_E_ARG;
+    if (!t->tracked) return TPC_E_STATE;
+    cudaStream_t s = t->stream;
+    if (!t->evM0) { CUDA_TRY(t, cudaEventCreate(&t->evM0)); CUDA_TRY(t, cudaEventCreate(&t->evM1)); }
+    DevParams dp; dp.P = t->P; dp.CB = t->CB; dp.nSec = t->nSec; dp.nRows = t->nRows;
+    const MergePtrs m = t->mp;
+    const int perSide = t->nSec >= 36 ? 18 : t->nSec;       // sectors per TPC side (tpctrk.h)
+    const float cosB = (float)std::cos((double)t->sectorDphi), sinB = (float)std::sin((double)t->sectorDphi);
+    const int grid = t->k6Blocks;                            // grid-stride over the tracks (their number is on the device)
+    CUDA_TRY(t, cudaEventRecord(t->evM0, s));
+    k7_init<<<grid, kK7Threads, 0, s>>>(m, t->nRows);
+    k7_hist<<<grid, kK7Threads, 0, s>>>(m, t->nRows);
+    k7_scan<<<1, 1024, 0, s>>>(m);
+    k7_scatter<<<grid, kK7Threads, 0, s>>>(m, t->nRows);
+    k7_match<<<grid, kK7Threads, 0, s>>>(m, dp, perSide, cosB, sinB);
+    k7_link<<<grid, kK7Threads, 0, s>>>(m);
+    k7_chains<<<grid, kK7Threads, 0, s>>>(m);
+    CUDA_TRY(t, cudaEventRecord(t->evM1, s));
+    CUDA_TRY(t, cudaGetLastError());
+    t->merged = true; t->mergeFetched = false;
+    return TPC_OK;
+}
+
+int tpc_get_merged(tpc_tracker* t, const int32_t** next, const int32_t** prev, const float** chi2, int32_t* n_tracks,
+                   const tpc_merged_track** merged, int32_t* n_merged, const int32_t** segments) {
+    if (!t) return TPC_E_ARG;
+    if (!t->merged) return TPC_E_STATE;
+    int rc = tpc_sync(t);                     // the track counters (the merge kernels are behind them on the stream)
+    if (rc != TPC_OK) return rc;
+    const int64_t nT = t->counters[kNTracks];
+    if (!t->mergeFetched) {
+        if (nT + 1 > t->outMergeCap) {
+            for (void* q : {(void*)t->outNext, (void*)t->outPrev, (void*)t->outMChi2, (void*)t->outMerged, (void*)t->outSegments})
+                if (q) cudaFreeHost(q);
+            const int64_t cap = std::max<int64_t>(nT + 1, 1024) * 3 / 2;
+            CUDA_TRY(t, cudaMallocHost(&t->outNext, 4 * cap)); CUDA_TRY(t, cudaMallocHost(&t->outPrev, 4 * cap));
+            CUDA_TRY(t, cudaMallocHost(&t->outMChi2, 4 * cap)); CUDA_TRY(t, cudaMallocHost(&t->outMerged, sizeof(tpc_merged_track) * cap));
+            CUDA_TRY(t, cudaMallocHost(&t->outSegments, 4 * cap));
+            if (!t->outMCount) CUDA_TRY(t, cudaMallocHost(&t->outMCount, 16));
+            t->outMergeCap = cap;
+        }
+        cudaStream_t s = t->stream;
+        const MergePtrs& m = t->mp;
+        CUDA_TRY(t, cudaMemcpyAsync(t->outMCount, m.mcount, 8, cudaMemcpyDeviceToHost, s));
+        if (nT) {
+            CUDA_TRY(t, cudaMemcpyAsync(t->outNext, m.next, 4 * nT, cudaMemcpyDeviceToHost, s));
+            CUDA_TRY(t, cudaMemcpyAsync(t->outPrev, m.prev, 4 * nT, cudaMemcpyDeviceToHost, s));
+            CUDA_TRY(t, cudaMemcpyAsync(t->outMChi2, m.chi2, 4 * nT, cudaMemcpyDeviceToHost, s));
+            CUDA_TRY(t, cudaMemcpyAsync(t->outMerged, m.merged, sizeof(tpc_merged_track) * nT, cudaMemcpyDeviceToHost, s));
+            CUDA_TRY(t, cudaMemcpyAsync(t->outSegments, m.segments, 4 * nT, cudaMemcpyDeviceToHost, s));
+        }
+        CUDA_TRY(t, cudaStreamSynchronize(s));
+        t->nMerged = (int32_t)t->outMCount[0];
+        t->nMergeLinks = (int32_t)(nT - t->nMerged);
+        float ms = 0.f;
+        CUDA_TRY(t, cudaEventElapsedTime(&ms, t->evM0, t->evM1));
+        t->mergeUs = ms * 1000.f;
+        t->mergeFetched = true;
+    }
+    if (next) *next = t->outNext;
+    if (prev) *prev = t->outPrev;
+    if (chi2) *chi2 = t->outMChi2;
+    if (n_tracks) *n_tracks = (int32_t)nT;
+    if (merged) *merged = t->outMerged;
+    if (n_merged) *n_merged = t->nMerged;
+    if (segments) *segments = t->outSegments;
     return TPC_OK;
 }
 
@@ -717,6 +815,7 @@ int tpc_get_stats(tpc_tracker* t, tpc_stats* out) {
     out->max_tracklets = t->ws ? t->dev.maxTracklets : 0;
     out->workspace_bytes_used = (int64_t)t->L.total;
     out->n_output_refetches = t->nRefetch;
+    if (t->mergeFetched) { out->merge_us = t->mergeUs; out->n_merged_tracks = t->nMerged; out->n_merge_links = t->nMergeLinks; }
     if (!t->tracked) return TPC_OK;
     out->n_links = t->counters[kNLinks];
     out->n_start_hits = t->counters[kNStart];

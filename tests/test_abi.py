@@ -27,8 +27,8 @@ def test_library_exports_every_declared_symbol():
 
 
 def test_struct_layouts_match_header():
-    assert ctypes.sizeof(binding.tpc_params) == 17 * 4
-    assert ctypes.sizeof(binding.tpc_stats) == 11 * 8 + 8 * 4
+    assert ctypes.sizeof(binding.tpc_params) == 19 * 4
+    assert ctypes.sizeof(binding.tpc_stats) == 11 * 8 + 4 * 4 + 8 * 4
     assert binding.TRACK_DTYPE.itemsize == 112
     p = binding.default_params()
     assert abs(p.err2_y - 0.01) < 1e-9 and p.min_hits == 10 and p.max_gap == 4 and p.seed_min_chain == 3

@@ -643,3 +643,100 @@ def test_neighbour_staging_in_shared_memory_changes_no_result(cfg, seed, scale):
     trk.set_neighbour_staging(False)
     run_gpu(ev, tracker=trk)
     assert np.array_equal(trk.debug_dump(binding.TPC_DUMP_LINKS), links_staged)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Phase II, first step: track merging (K7) against the oracle's S7
+
+def _merge_oracle_params(params=None):
+    """Oracle parameters with the sector angle the CUDA path gets through the C ABI (a float)."""
+    p = params or oracle.default_params()
+    p.sector_dphi = float(np.float32(np.deg2rad(20.0)))
+    return p
+
+
+def _compare_merge(ev, trk, tracks, ids, ref):
+    """next / prev / chi2 of the CUDA path against the oracle's, tracks keyed by their first cluster id."""
+    g = trk.get_merged()
+    key_g = ids[tracks["cluster_offset"]].astype(np.int64)
+    key_o = ref.cluster_ids[ref.tracks["cluster_offset"]].astype(np.int64)
+    assert np.array_equal(np.sort(key_g), np.sort(key_o))
+    pos_o = {int(k): i for i, k in enumerate(key_o)}
+    to_o = np.array([pos_o[int(k)] for k in key_g])                 # GPU track index -> oracle track index
+    nxt_g = np.where(g["next"] >= 0, to_o[np.maximum(g["next"], 0)], -1)
+    prv_g = np.where(g["prev"] >= 0, to_o[np.maximum(g["prev"], 0)], -1)
+    nxt_o, prv_o = ref.merge_next[to_o], ref.merge_prev[to_o]
+    bad = np.nonzero((nxt_g != nxt_o) | (prv_g != prv_o))[0]
+    tie = ref.merge_tie[to_o] == 1
+    # a decision may differ only where the oracle flagged chi2 values within 1e-6 relative (of the cut or of each other)
+    partner_tie = np.zeros_like(tie)
+    for arr in (nxt_o, prv_o, nxt_g, prv_g):
+        partner_tie |= (arr >= 0) & (ref.merge_tie[np.maximum(arr, 0)] == 1)
+    assert np.all(tie[bad] | partner_tie[bad]), f"{bad.size} merge decisions differ without a near-tie"
+    same = (nxt_g == nxt_o) & (nxt_o >= 0)
+    a, b = g["chi2"][same].astype(np.float64), ref.merge_chi2[to_o][same]
+    assert np.all(np.abs(a - b) <= 1e-5 + 1e-4 * np.abs(b)), np.abs(a - b).max()
+    # merged-track records: chains consistent with next/prev, every track in exactly one
+    m, seg = g["merged"], g["segments"]
+    assert m.size == tracks.size - int((g["next"] >= 0).sum()) and int(m["n_segments"].sum()) == tracks.size
+    assert np.array_equal(np.sort(seg), np.arange(tracks.size))
+    for r in m[:: max(1, m.size // 3000)]:
+        chain = seg[r["segment_offset"]: r["segment_offset"] + r["n_segments"]]
+        assert chain[0] == r["first_track"] and g["prev"][chain[0]] == -1 and g["next"][chain[-1]] == -1
+        assert np.array_equal(g["next"][chain[:-1]], chain[1:])
+        assert r["n_clusters"] == int(tracks["n_clusters"][chain].sum())
+    return {"links": int((g["next"] >= 0).sum()), "differ": int(bad.size), "near_tie_tracks": int(tie.sum()),
+            "bitexact_chi2": bool(np.array_equal(a.astype(np.float32), b.astype(np.float32)))}
+
+
+@pytest.mark.parametrize("cfg,seed", [(1, 0), (2, 0), (2, 5), (3, 0)])
+def test_track_merging_matches_the_oracle(cfg, seed, capsys):
+    """tpc_merge_tracks (K7) on the tracks of configs 1-3: every link (which segment continues which, from both ends)
+    equals the oracle's S7 except at flagged near-ties, chi2 within 1e-4 rel / 1e-5 abs, merged records consistent."""
+    _cuda()
+    ev = datagen.config_event(cfg, seed=seed)
+    o = oracle.Oracle(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz, _merge_oracle_params())
+    ref = o.merge(o.run(ev.row_counts, ev.y, ev.z))
+    trk, tracks, ids = run_gpu(ev)
+    trk.merge_tracks()
+    out = _compare_merge(ev, trk, tracks, ids, ref)
+    st = trk.get_stats()
+    assert st["n_merge_links"] == out["links"] and st["n_merged_tracks"] == tracks.size - out["links"] and st["merge_us"] > 0
+    if cfg >= 2:
+        assert out["links"] > 50
+    with capsys.disabled():
+        print(f"\n[merge config {cfg} seed {seed}] tracks {tracks.size} {out} K7 {st['merge_us']:.1f} us")
+
+
+def test_track_merging_hand_made_cases_and_parameters():
+    """A helix crossing a sector border and a track with a 12-row hole (tests/test_oracle_merge.py's cases) through the
+    CUDA path; merge_max_row_gap and merge_chi2 are applied; merging twice gives the same; no tracks, no links."""
+    torch = _cuda()
+    from test_oracle_merge import hits_of_global_helix, BZ
+    rng = np.random.default_rng(8)
+    rx = datagen.default_row_x()
+    hits = hits_of_global_helix(rng, 0.6, 1, 1.2, 0.5, 0.1) + hits_of_global_helix(rng, 2.0, -1, 4.0, -0.3, 0.1, skip=lambda s, r: 60 <= r < 72)
+    ev = datagen.event_from_hits(hits, 36, rx, BZ)
+    for gap, chi in ((40, 50.0), (12, 50.0), (40, 1e-6)):
+        po, pg = _merge_oracle_params(), binding.default_params()
+        po.merge_max_row_gap = pg.merge_max_row_gap = gap
+        po.merge_chi2 = pg.merge_chi2 = chi
+        o = oracle.Oracle(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz, po)
+        ref = o.merge(o.run(ev.row_counts, ev.y, ev.z))
+        trk, tracks, ids = run_gpu(ev, pg)
+        trk.merge_tracks()
+        out = _compare_merge(ev, trk, tracks, ids, ref)
+        assert out["differ"] == 0
+        if (gap, chi) == (40, 50.0):
+            assert out["links"] >= 2                      # the border crossing and the hole
+            first = trk.get_merged()
+            trk.merge_tracks()
+            again = trk.get_merged()
+            assert all(np.array_equal(first[k], again[k]) for k in ("next", "prev", "chi2"))
+        if chi < 1e-3:
+            assert out["links"] == 0
+    empty = datagen.event_from_hits([], 36, rx, BZ)
+    trk, tracks, ids = run_gpu(empty, max_clusters=16)
+    trk.merge_tracks()
+    g = trk.get_merged()
+    assert g["next"].size == 0 and g["merged"].size == 0
