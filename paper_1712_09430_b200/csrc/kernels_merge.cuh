@@ -153,11 +153,14 @@ __device__ __forceinline__ unsigned long long k7_pack(float chi2, uint32_t key) 
     return ((unsigned long long)__float_as_uint(chi2) << 32) | (unsigned long long)key;
 }
 
-// One thread per segment A: its best outer partner, and A's bid for being the best inner partner of every match.
+// One WARP per segment A (its candidates - a few to a few dozen - are shared out over the lanes): A's best outer
+// partner, and A's bid for being the best inner partner of every match.
 __global__ void __launch_bounds__(kK7Threads) k7_match(MergePtrs m, DevParams dp, int perSide, float cosB, float sinB) {
     const unsigned nT = m.counters[kNTracks];
     const int nRows = dp.nRows;
-    for (unsigned a = blockIdx.x * kK7Threads + threadIdx.x; a < nT; a += gridDim.x * kK7Threads) {
+    const unsigned lane = threadIdx.x & 31u;
+    const unsigned warp = (blockIdx.x * kK7Threads + threadIdx.x) >> 5, nWarps = (gridDim.x * kK7Threads) >> 5;
+    for (unsigned a = warp; a < nT; a += nWarps) {
         const tpc_track TA = m.tracks[a];
         const int side = TA.sector / perSide, sa = TA.sector - side * perSide;
         const uint32_t keyA = m.key[a];
@@ -175,6 +178,8 @@ __global__ void __launch_bounds__(kK7Threads) k7_match(MergePtrs m, DevParams dp
                 if (sb < 0) sb += perSide;
                 if (sb >= perSide) sb -= perSide;
                 const int secB = side * perSide + sb;
+                const unsigned j0 = m.binStart[secB * nRows + rLo], j1 = m.binStart[secB * nRows + rHi + 1];
+                if (j0 >= j1) continue;
                 int dsec = sb - sa;
                 if (dsec > perSide / 2) dsec -= perSide;
                 if (dsec < -perSide / 2) dsec += perSide;
@@ -186,9 +191,8 @@ __global__ void __launch_bounds__(kK7Threads) k7_match(MergePtrs m, DevParams dp
                 st.c13 = TA.c[13]; st.c14 = TA.c[14];
                 float xA = TA.x;
                 if (dsec != 0 && !k7_rotate(st, xA, cosB, dsec > 0 ? sinB : -sinB, dp.CB, dp.P.kf_smax)) continue;
-                const unsigned j0 = m.binStart[secB * nRows + rLo], j1 = m.binStart[secB * nRows + rHi + 1];
 #pragma unroll 1
-                for (unsigned j = j0; j < j1; j++) {
+                for (unsigned j = j0 + lane; j < j1; j += 32u) {
                     const unsigned b = m.order[j];
                     if (b == a) continue;
                     const tpc_track TB = m.tracks[b];
@@ -206,8 +210,19 @@ __global__ void __launch_bounds__(kK7Threads) k7_match(MergePtrs m, DevParams dp
                 }
             }
         }
-        m.out[a] = best;
-        m.outChi2[a] = bestC;
+        // the warp's best: smaller chi2, then smaller key (lanes without a match carry the largest possible word)
+        unsigned long long w = best >= 0 ? k7_pack(bestC, bestKey) : ~0ull;
+        int wb = best;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const unsigned long long w2 = __shfl_xor_sync(0xffffffffu, w, o);
+            const int b2 = __shfl_xor_sync(0xffffffffu, wb, o);
+            if (w2 < w) { w = w2; wb = b2; }
+        }
+        if (lane == 0) {
+            m.out[a] = wb;
+            m.outChi2[a] = wb >= 0 ? __uint_as_float((unsigned)(w >> 32)) : 0.f;
+        }
     }
 }
 // A link survives if it is mutual.
