@@ -452,6 +452,19 @@ def main():
     st = trk.get_stats()
     value, ms, n_total = aggregate(dist, dev, ev.n_clusters, step_ms)
 
+    # ---- Phase II track merging (K7; extra key, not part of the metric): device time of
+    # tpc_merge_tracks on the tracks of this event, L2 flushed before, CUDA events inside the library
+    merge_us = []
+    for _ in range(max(3, min(args.steps, 10))):
+        flush.fill_(1)
+        trk.track_sectors()
+        trk.merge_tracks()
+        trk.get_merged()
+        merge_us.append(trk.get_stats()["merge_us"])
+    stm = trk.get_stats()
+    merge_leg = {"kernel": "K7 track merging (tpc_merge_tracks: 7 launches)", "us": round(sum(merge_us[1:]) / len(merge_us[1:]), 1),
+                 "n_tracks": stm["n_tracks"], "n_links": stm["n_merge_links"], "n_merged_tracks": stm["n_merged_tracks"]}
+
     # ---- end to end through the C ABI with HOST buffers (pinned), H2D + D2H of every step inside the timed region.
     # ONE host thread keeps n_pipe tracker instances (each on its own stream) in flight, round robin: for the oldest
     # instance tpc_get_tracks (waits once: the download was queued behind its kernels), then
@@ -553,6 +566,7 @@ def main():
     }
     if roof_issue:
         out["roofline_issue"] = roof_issue
+    out["merge"] = merge_leg
     if args.events_per_call > 1 and args.config <= 3:
         me = multi_event_leg(torch, binding, datagen, args, params, dev, rank, args.events_per_call, max(3, min(args.steps, 10)))
         me["value"] = reduce_over_ranks(dist, me["value"], "sum", dev)      # whole job: sum of the ranks' rates
