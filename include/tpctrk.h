@@ -230,6 +230,12 @@ int tpc_get_merged(tpc_tracker* t, const int32_t** next, const int32_t** prev, c
 size_t tpc_debug_dump_bytes(tpc_tracker* t, int stage);
 int tpc_debug_dump(tpc_tracker* t, int stage, void* host_dst, size_t bytes);
 
+/* Memory-safety check of the kernels (tests; compute-sanitizer is not available on the target pool): every buffer of
+ * the workspace is followed by a 256-byte guard zone that tpc_set_workspace fills with a pattern.  Synchronises and
+ * returns the number of guard zones that have been written to since (0 = no kernel wrote past the end of a buffer),
+ * or a negative tpc_error. */
+int tpc_debug_check_guards(tpc_tracker* t);
+
 const char* tpc_strerror(int code);
 int tpc_last_cuda_error(const tpc_tracker* t);
 /* Number of kernel launches one tpc_track_sectors enqueues (for bench.py's gpu_launches). */

@@ -103,6 +103,7 @@ def lib():
         L.tpc_debug_dump_bytes.argtypes = [vp, i32]
         L.tpc_debug_dump_bytes.restype = ctypes.c_size_t
         L.tpc_debug_dump.argtypes = [vp, i32, vp, ctypes.c_size_t]
+        L.tpc_debug_check_guards.argtypes = [vp]
         L.tpc_strerror.argtypes = [i32]
         L.tpc_strerror.restype = ctypes.c_char_p
         L.tpc_last_cuda_error.argtypes = [vp]
@@ -269,6 +270,12 @@ class Tracker:
         d["total_us"] = float(s.kernel_us[6])
         d["k6a_fused"] = bool(s.kernel_us[7] > 0.5)
         return d
+
+    def debug_check_guards(self) -> int:
+        rc = int(self._L.tpc_debug_check_guards(self._h))
+        if rc < 0:
+            self._check(rc, "tpc_debug_check_guards")
+        return rc
 
     def launches_per_track(self) -> int:
         return int(self._L.tpc_launches_per_track(self._h))

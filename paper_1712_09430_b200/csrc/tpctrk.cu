@@ -27,6 +27,9 @@ struct Layout {   // byte offsets into the workspace
         tracks, clusterIds, counters, sectorGidBase,
         mKey, mBinStart, mBinCursor, mOrder, mBestIn, mOut, mOutChi2, mNext, mPrev, mChi2, mMerged, mSegments, mCount, total;
     int64_t hitCap, binCap, maxTracklets;
+    enum : int { kMaxGuards = 64 };
+    size_t guard[kMaxGuards];        // offsets of the guard zones behind the buffers
+    int nGuards;
 };
 
 }  // namespace
@@ -105,7 +108,16 @@ Layout make_layout(const tpc_tracker* t, int64_t maxClusters) {
     L.binCap = (int64_t)((double)maxClusters * (double)t->P.grid_bins_per_hit) + 2 * NR + 16;
     L.maxTracklets = (int64_t)((double)maxClusters * (double)t->P.max_tracklets_per_cluster) + 4096;
     size_t o = 0;
-    auto take = [&](size_t bytes) { size_t r = o; o = align_up(o + bytes); return r; };
+    L.nGuards = 0;
+    // every buffer is followed by a 256-byte guard zone (filled with a pattern by tpc_set_workspace, checked by
+    // tpc_debug_check_guards: compute-sanitizer is not available on the target pool)
+    auto take = [&](size_t bytes) {
+        size_t r = o;
+        o = align_up(o + bytes);
+        if (L.nGuards < Layout::kMaxGuards) L.guard[L.nGuards++] = o;
+        o += kAlign;
+        return r;
+    };
     L.inY = take(sizeof(float) * (maxClusters + 16));
     L.inZ = take(sizeof(float) * (maxClusters + 16));
     L.grid = take(sizeof(RowGrid) * (NR + 2));
@@ -544,6 +556,8 @@ int tpc_set_workspace(tpc_tracker* t, void* dev_ptr, size_t bytes) {
     t->ws = (char*)dev_ptr; t->wsBytes = bytes; t->maxClusters = lo;
     t->L = make_layout(t, lo);
     bind_pointers(t);
+    for (int g = 0; g < t->L.nGuards; g++)
+        CUDA_TRY(t, cudaMemsetAsync(t->ws + t->L.guard[g], 0xA5, kAlign, t->stream));
     CUDA_TRY(t, cudaMemcpyAsync((void*)t->dev.rowX, t->rowX.data(), sizeof(float) * t->nRows, cudaMemcpyHostToDevice, t->stream));
     CUDA_TRY(t, cudaStreamSynchronize(t->stream));
     if (!t->haveEvents) {
@@ -884,6 +898,19 @@ int tpc_debug_dump(tpc_tracker* t, int stage, void* host_dst, size_t bytes) {
     if ((e = cudaGetLastError()) != cudaSuccess) fail(e);
     cudaFree(tmp);
     return rc;
+}
+
+int tpc_debug_check_guards(tpc_tracker* t) {
+    if (!t) return TPC_E_ARG;
+    if (!t->ws) return TPC_E_STATE;
+    CUDA_TRY(t, cudaStreamSynchronize(t->stream));
+    std::vector<unsigned char> h(kAlign);
+    int bad = 0;
+    for (int g = 0; g < t->L.nGuards; g++) {
+        CUDA_TRY(t, cudaMemcpy(h.data(), t->ws + t->L.guard[g], kAlign, cudaMemcpyDeviceToHost));
+        for (unsigned char c : h) if (c != 0xA5) { bad++; break; }
+    }
+    return bad;      // number of guard zones that were written to
 }
 
 const char* tpc_strerror(int code) {

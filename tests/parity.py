@@ -95,4 +95,7 @@ def compare(ev, trk, tracks, ids, ref, rtol=1e-4, atol=1e-5, check_links=True):
         assert np.array_equal(np.sort(ids.astype(np.int64)), np.sort(ref.cluster_ids.astype(np.int64)))
     out["n_tracks"] = int(tracks.size)
     out["n_tracklets"] = int(recs.size)
+    # no kernel wrote past the end of any workspace buffer (guard zones behind every buffer; tpctrk.h)
+    out["guards_hit"] = trk.debug_check_guards()
+    assert out["guards_hit"] == 0, f"{out['guards_hit']} workspace guard zones overwritten"
     return out

@@ -65,6 +65,7 @@ def test_time_frame_full_size_sampled_sectors():
     # properties that hold at any size
     assert np.unique(ids).size == ids.size                       # one track hypothesis at most per hit
     assert tracks["n_clusters"].min() >= 10
+    assert trk.debug_check_guards() == 0                         # no buffer overrun at the largest size either
     sec_of = np.repeat(np.arange(ev.n_sectors * ev.n_rows), ev.row_counts.reshape(-1))
     base = ev.row_base
     for s in (3, 25):
@@ -685,6 +686,7 @@ def _compare_merge(ev, trk, tracks, ids, ref):
         assert chain[0] == r["first_track"] and g["prev"][chain[0]] == -1 and g["next"][chain[-1]] == -1
         assert np.array_equal(g["next"][chain[:-1]], chain[1:])
         assert r["n_clusters"] == int(tracks["n_clusters"][chain].sum())
+    assert trk.debug_check_guards() == 0          # K7 wrote past the end of none of its buffers
     return {"links": int((g["next"] >= 0).sum()), "differ": int(bad.size), "near_tie_tracks": int(tie.sum()),
             "bitexact_chi2": bool(np.array_equal(a.astype(np.float32), b.astype(np.float32)))}
 
