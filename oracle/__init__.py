@@ -28,6 +28,7 @@ class Params(ctypes.Structure):
         ("pad", ctypes.c_int32),
         ("merge_chi2", ctypes.c_double), ("merge_max_row_gap", ctypes.c_int32), ("pad2", ctypes.c_int32),
         ("sector_dphi", ctypes.c_double),
+        ("field_ar", ctypes.c_double), ("field_az", ctypes.c_double), ("ms_x0_inv", ctypes.c_double),
     ]
 
 
@@ -36,6 +37,9 @@ TRACKLET_DTYPE = np.dtype([
     ("first_row", np.int32), ("last_row", np.int32), ("kept", np.int32), ("n_fit", np.int32),
     ("near_tie", np.int32), ("x", np.float64), ("p", np.float64, 5), ("c", np.float64, 15),
     ("chi2", np.float64)], align=True)
+REFIT_DTYPE = np.dtype([
+    ("first_track", np.int32), ("sector", np.int32), ("n_fit", np.int32), ("ok", np.int32),
+    ("x", np.float64), ("p", np.float64, 5), ("c", np.float64, 15), ("chi2", np.float64)], align=True)
 TRACK_DTYPE = np.dtype([
     ("start_gid", np.int64), ("cluster_offset", np.int64), ("sector", np.int32), ("n_clusters", np.int32),
     ("first_row", np.int32), ("last_row", np.int32), ("n_fit", np.int32), ("pad", np.int32),
@@ -88,6 +92,11 @@ def lib():
         L.oracle_n_merged.restype = i64
         L.oracle_n_merged.argtypes = [vp]
         L.oracle_get_merge.argtypes = [vp] + [vp] * 6
+        L.oracle_scatter.argtypes = [vp, vp, dbl, dbl]
+        L.oracle_refit.argtypes = [vp]
+        L.oracle_sizeof_refit.restype = i32
+        L.oracle_get_refits.argtypes = [vp, vp]
+        assert L.oracle_sizeof_refit() == REFIT_DTYPE.itemsize, (L.oracle_sizeof_refit(), REFIT_DTYPE.itemsize)
         L.oracle_rotate.restype = i32
         L.oracle_rotate.argtypes = [i32, vp, vp, vp, dbl, dbl, dbl]
         L.oracle_chi2_5.restype = dbl
@@ -151,6 +160,14 @@ class Oracle:
                            res.merge_tie.ctypes.data, res.merged_offset.ctypes.data, res.merged_segs.ctypes.data)
         return res
 
+    def refit(self, res: "Result") -> "Result":
+        """Final fit of the merged tracks (S8) after merge(); adds res.refits (one per merged track)."""
+        L, h = lib(), self._h
+        L.oracle_refit(h)
+        res.refits = np.empty(res.merged_offset.size - 1, dtype=REFIT_DTYPE)
+        L.oracle_get_refits(h, res.refits.ctypes.data)
+        return res
+
     def stage_seconds(self):
         s = np.zeros(6)
         lib().oracle_get_stage_seconds(self._h, s.ctypes.data)
@@ -195,6 +212,19 @@ def run_event_merged(ev, params: Params | None = None, precision="float") -> Res
     """Phase I + Phase II merging on a datagen.Event-like object."""
     o = Oracle(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz, params, precision)
     return o.merge(o.run(ev.row_counts, ev.y, ev.z))
+
+
+def run_event_refit(ev, params: Params | None = None, precision="float") -> Result:
+    """Phase I + Phase II (merging, final fit)."""
+    o = Oracle(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz, params, precision)
+    return o.refit(o.merge(o.run(ev.row_counts, ev.y, ev.z)))
+
+
+def scatter(p, c, length, x0_inv):
+    """Covariance c[15] after multiple scattering over `length` cm (S8 process noise); returns the new c."""
+    pa, ca = np.array(p, dtype=np.float64), np.array(c, dtype=np.float64).copy()
+    lib().oracle_scatter(pa.ctypes.data, ca.ctypes.data, float(length), float(x0_inv))
+    return ca
 
 
 def rotate(x, p, c, beta, cb, smax=0.95, precision="double"):

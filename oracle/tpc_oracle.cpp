@@ -49,6 +49,8 @@ struct ParamsD {                 /* DESIGN.md "Constants" */
     int32_t merge_max_row_gap;   /* S7: max pad rows between the end of the inner and the start of the outer segment */
     int32_t pad2;
     double sector_dphi;          /* S7: angle between neighbouring sector frames [rad] */
+    double field_ar, field_az;   /* S8: Bz(r, z) = Bz * (1 + field_ar * r^2 + field_az * z^2)  [1/cm^2] */
+    double ms_x0_inv;            /* S8: 1 / radiation length of the gas [1/cm]; 0 = no multiple scattering */
 };
 
 /* ------------------------------------------------------------------ track model (S5) */
@@ -602,6 +604,93 @@ template <class T> struct Tracker {
         }
     }
 
+    /* ---------------------------------------------------------------- S8 final fit of the merged tracks (Phase II) */
+    /* "the full track is refit using the full Kalman filter.  A polynomial approximation of the magnetic
+     * field avoids the slow memory access to a field map."  Reading R-17 (S8): one inward filter pass over ALL
+     * clusters of a merged track, from its outermost cluster to its innermost one, across the sector frames of its
+     * segments; per step the field is the polynomial evaluated at the state's point, and multiple scattering over the
+     * step's path is added to the covariance. */
+    struct RefitOut { int32_t first_track, sector, n_fit, ok; double x, p[5], c[15], chi2; };
+    std::vector<RefitOut> refits;           /* one per merged track, in the order of mergedOffset */
+
+    int rowOfCluster(int64_t g) const {
+        const int sr = int(std::upper_bound(rowBase.begin(), rowBase.end(), g) - rowBase.begin()) - 1;
+        return sr % nRows;
+    }
+    T fieldCB(const State<T> &st) const {   /* curvature constant with the field at the state's point */
+        const T r2 = st.x * st.x + st.p[0] * st.p[0];
+        return CB * (T(1) + T(pd.field_ar) * r2 + T(pd.field_az) * (st.p[1] * st.p[1]));
+    }
+    /* multiple scattering over a straight path of length L (Highland without the log term, beta = 1):
+     * theta0^2 = (0.0136 GeV / p)^2 L / X0, 1/p = |k| / sqrt(1 + t^2); projected on (sin phi, dz/ds, q/pT) */
+    void addScattering(State<T> &st, T L) const {
+        if (!(pd.ms_x0_inv > 0.0)) return;
+        const T s = st.p[2], t = st.p[3], k = st.p[4];
+        const T one_t2 = T(1) + t * t;
+        const T th2 = (T(0.0136) * T(0.0136)) * ((k * k) / one_t2) * (L * T(pd.ms_x0_inv));
+        st.C[2][2] = st.C[2][2] + (th2 * (T(1) - s * s)) * one_t2;
+        st.C[3][3] = st.C[3][3] + (th2 * one_t2) * one_t2;
+        const T c43 = ((th2 * t) * k) * one_t2;
+        st.C[4][3] = st.C[4][3] + c43; st.C[3][4] = st.C[4][3];
+        st.C[4][4] = st.C[4][4] + ((th2 * t) * t) * (k * k);
+    }
+
+    void refitMerged() {
+        refits.clear();
+        const int perSide = nSec >= 36 ? 18 : nSec;
+        for (size_t m = 0; m + 1 < mergedOffset.size(); m++) {
+            const int s0 = mergedOffset[m], s1 = mergedOffset[m + 1];
+            const TrackOut &inner = tracks[mergedSegs[s0]];
+            RefitOut o; std::memset(&o, 0, sizeof(o));
+            o.first_track = mergedSegs[s0]; o.sector = inner.sector;
+            /* default output: the innermost segment's Phase-I state (kept if the refit cannot be done) */
+            o.x = inner.x; o.chi2 = inner.chi2; o.n_fit = 0; o.ok = 0;
+            std::memcpy(o.p, inner.p, sizeof(o.p)); std::memcpy(o.c, inner.c, sizeof(o.c));
+            /* start: the outermost segment's state taken to the pad row of its outermost cluster */
+            const TrackOut &outer = tracks[mergedSegs[s1 - 1]];
+            State<T> st; st.x = T(outer.x); st.chi2 = T(0); st.nfit = 0;
+            for (int i = 0; i < 5; i++) st.p[i] = T(outer.p[i]);
+            for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) st.C[i][j] = T(0);
+            bool ok = propagate(st, rowX[outer.last_row], fieldCB(st), smax);
+            int curSector = outer.sector;
+            bool first = true;
+            for (int sg = s1 - 1; ok && sg >= s0; sg--) {
+                const TrackOut &seg = tracks[mergedSegs[sg]];
+                for (int c = seg.n_clusters - 1; ok && c >= 0; c--) {
+                    const int64_t g = clusterIds[seg.cluster_offset + c];
+                    const int row = rowOfCluster(g);
+                    if (first) {           /* the outermost cluster is the starting point, not a measurement */
+                        st.p[0] = y[g]; st.p[1] = z[g]; st.x = rowX[row];
+                        initCov(st); st.chi2 = T(0); st.nfit = 0;
+                        first = false;
+                        continue;
+                    }
+                    if (seg.sector != curSector) {   /* into the next segment's sector frame (S7 rotation) */
+                        int dsec = seg.sector % perSide - curSector % perSide;
+                        if (dsec > perSide / 2) dsec -= perSide;
+                        if (dsec < -perSide / 2) dsec += perSide;
+                        const double beta = double(dsec) * pd.sector_dphi;
+                        ok = rotate(st, T(std::cos(beta)), T(std::sin(beta)), fieldCB(st), smax);
+                        curSector = seg.sector;
+                        if (!ok) break;
+                    }
+                    const T x0 = st.x, y0 = st.p[0], z0 = st.p[1];
+                    ok = propagate(st, rowX[row], fieldCB(st), smax);
+                    if (!ok) break;
+                    const T dx = st.x - x0, dy = st.p[0] - y0, dz = st.p[1] - z0;
+                    addScattering(st, std::sqrt((dx * dx + dy * dy) + dz * dz));
+                    update_hit(st, y[g], z[g], err2y, err2z);
+                }
+            }
+            if (ok && !first) {
+                o.ok = 1; o.x = double(st.x); o.chi2 = double(st.chi2); o.n_fit = st.nfit; o.sector = curSector;
+                for (int i = 0; i < 5; i++) o.p[i] = double(st.p[i]);
+                for (int i = 0, k = 0; i < 5; i++) for (int j = 0; j <= i; j++) o.c[k++] = double(st.C[i][j]);
+            }
+            refits.push_back(o);
+        }
+    }
+
     void run(const int32_t *rowCounts, const float *yin, const float *zin, int bruteForce) {
         using clk = std::chrono::steady_clock;
         brute = bruteForce != 0;
@@ -679,6 +768,7 @@ void oracle_default_params(ParamsD *p) {
     p->max_gap = 4; p->min_hits = 10; p->seed_min_chain = 3; p->pad = 0;
     p->merge_chi2 = 50.0; p->merge_max_row_gap = 40; p->pad2 = 0;
     p->sector_dphi = 20.0 * 3.14159265358979323846 / 180.0;
+    p->field_ar = 0.0; p->field_az = 0.0; p->ms_x0_inv = 0.0;
 }
 
 void *oracle_create(int n_sectors, int n_rows, const float *row_x, double bz, const ParamsD *p, int use_double) {
@@ -761,6 +851,24 @@ void oracle_get_merge(void *hv, int32_t *next, int32_t *prev, double *chi2, uint
         std::memcpy(merged_segs, t.mergedSegs.data(), t.mergedSegs.size() * 4);
     };
     if (h->useDouble) cp(*h->d); else cp(*h->f);
+}
+/* primitive for the pins: covariance after multiple scattering over a path L [cm] in a gas of radiation length 1/x0_inv */
+void oracle_scatter(const double *p, double *c, double L, double x0_inv) {
+    ParamsD pd; oracle_default_params(&pd); pd.ms_x0_inv = x0_inv;
+    const float rx[3] = {1.f, 2.f, 3.f};
+    Tracker<double> t(1, 3, rx, 0.5, pd);
+    State<double> st; st.x = 0; st.chi2 = 0; st.nfit = 0;
+    for (int i = 0; i < 5; i++) st.p[i] = p[i];
+    for (int i = 0, k = 0; i < 5; i++) for (int j = 0; j <= i; j++) { st.C[i][j] = st.C[j][i] = c[k++]; }
+    t.addScattering(st, L);
+    for (int i = 0, k = 0; i < 5; i++) for (int j = 0; j <= i; j++) c[k++] = st.C[i][j];
+}
+void oracle_refit(void *hv) { Handle *h = (Handle *)hv; if (h->useDouble) h->d->refitMerged(); else h->f->refitMerged(); }
+int32_t oracle_sizeof_refit(void) { return (int32_t)sizeof(Tracker<float>::RefitOut); }
+void oracle_get_refits(void *hv, void *dst) {
+    Handle *h = (Handle *)hv;
+    if (h->useDouble) std::memcpy(dst, h->d->refits.data(), h->d->refits.size() * sizeof(Tracker<double>::RefitOut));
+    else std::memcpy(dst, h->f->refits.data(), h->f->refits.size() * sizeof(Tracker<float>::RefitOut));
 }
 /* primitives for the pins: rotate a state (x[1], p[5], c[15]) by beta; chi2 of d with covariance S (15) */
 int oracle_rotate(int use_double, double *x, double *p, double *c, double beta, double CB, double smax) {
