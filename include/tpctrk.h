@@ -61,6 +61,10 @@ typedef struct tpc_params {
     float merge_chi2;               /* Phase II merging: max chi2 (5 parameters) of two matching segments  50 */
     int32_t merge_max_row_gap;      /* ... max pad rows between the end of the inner segment and the
                                        start of the outer one                                              40 */
+    float field_ar, field_az;       /* final fit: Bz(r, z) = Bz (1 + field_ar r^2 + field_az z^2), the polynomial
+                                       field approximation of PAPER.md:46  [1/cm^2]                       0, 0 */
+    float ms_x0_inv;                /* final fit: 1 / radiation length of the gas [1/cm]; 0 = no multiple
+                                       scattering noise                                                     0 */
 } tpc_params;
 
 typedef struct tpc_geometry {
@@ -93,7 +97,7 @@ typedef struct tpc_stats {
                                  download queued by tpc_track_sectors was estimated too small */
     float merge_us;           /* device time of the last tpc_merge_tracks (K7), valid after tpc_get_merged */
     int32_t n_merged_tracks, n_merge_links;   /* after tpc_get_merged */
-    int32_t pad_;
+    float refit_us;           /* device time of the last tpc_refit_tracks (K8), valid after tpc_get_refit */
     float kernel_us[8];       /* K1 sort+grid, K2 neighbours, K3/K4 clean+start, K5 construct, K6a weights,
                                  K6b select+compact, [6] = K1..K6 total, [7] = 1.0 if the K6a weights pass of this
                                  event ran inside the K5 launch (about one tracklet per GPU thread or fewer: [3]
@@ -224,6 +228,27 @@ int tpc_merge_tracks(tpc_tracker* t);
  * pinned memory, valid until the next merge/track/reset/destroy.  Any output pointer may be NULL. */
 int tpc_get_merged(tpc_tracker* t, const int32_t** next, const int32_t** prev, const float** chi2, int32_t* n_tracks,
                    const tpc_merged_track** merged, int32_t* n_merged, const int32_t** segments);
+
+/* ---- Phase II, second step: final fit of the merged tracks (reading S8 of DESIGN.md) ----
+ * "the full track is refit using the full Kalman filter.  A polynomial approximation of the magnetic field avoids the
+ * slow memory access to a field map."  One inward filter pass over ALL clusters of a merged track, from its outermost
+ * cluster (the starting point) to its innermost one, across the sector frames of its segments; per step the field is
+ * the polynomial of tpc_params at the state's point, and multiple scattering over the step's path is added to the
+ * covariance (ms_x0_inv).  ok = 0: the pass could not be completed (|sin phi| limit); the record then repeats the
+ * innermost segment's Phase-I state with n_fit = 0. */
+typedef struct tpc_refit_track {
+    int32_t first_track;      /* innermost segment (track index as in tpc_get_tracks) = tpc_merged_track.first_track */
+    int32_t sector;           /* frame of the state */
+    int32_t n_fit;            /* clusters used as measurements (all but the outermost one) */
+    int32_t ok;
+    float x, p[5], c[15], chi2;
+} tpc_refit_track;
+
+/* Run the final fit (K8) on the merged tracks of the last tpc_merge_tracks, on the stream.  Asynchronous.
+ * TPC_E_STATE before tpc_merge_tracks. */
+int tpc_refit_tracks(tpc_tracker* t);
+/* Synchronise and download: refit[i] belongs to merged[i] of tpc_get_merged (same event).  Library-owned pinned memory. */
+int tpc_get_refit(tpc_tracker* t, const tpc_refit_track** refit, int32_t* n_merged);
 
 /* Stage parity hooks (tests): copy one stage's buffers, converted to canonical (load-index) form, to host_dst.
  * Synchronous; allocates temporary device memory.  bytes must equal tpc_debug_dump_bytes(t, stage). */

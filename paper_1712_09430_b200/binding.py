@@ -24,6 +24,7 @@ class tpc_params(ctypes.Structure):
         ("min_hits", ctypes.c_int32), ("seed_min_chain", ctypes.c_int32),
         ("max_tracklets_per_cluster", ctypes.c_float), ("grid_bins_per_hit", ctypes.c_float),
         ("merge_chi2", ctypes.c_float), ("merge_max_row_gap", ctypes.c_int32),
+        ("field_ar", ctypes.c_float), ("field_az", ctypes.c_float), ("ms_x0_inv", ctypes.c_float),
     ]
 
 
@@ -40,7 +41,7 @@ class tpc_stats(ctypes.Structure):
         ("n_tracklets", ctypes.c_int64), ("n_tracklet_hits", ctypes.c_int64), ("n_tracks", ctypes.c_int64),
         ("n_track_clusters", ctypes.c_int64), ("workspace_bytes_used", ctypes.c_int64),
         ("max_clusters", ctypes.c_int64), ("max_tracklets", ctypes.c_int64), ("n_output_refetches", ctypes.c_int64),
-        ("merge_us", ctypes.c_float), ("n_merged_tracks", ctypes.c_int32), ("n_merge_links", ctypes.c_int32), ("pad_", ctypes.c_int32),
+        ("merge_us", ctypes.c_float), ("n_merged_tracks", ctypes.c_int32), ("n_merge_links", ctypes.c_int32), ("refit_us", ctypes.c_float),
         ("kernel_us", ctypes.c_float * 8),
     ]
 
@@ -54,7 +55,9 @@ TRACKLET_DTYPE = np.dtype([
     ("first_row", np.int32), ("last_row", np.int32), ("n_fit", np.int32), ("x", np.float32),
     ("p", np.float32, 5), ("c", np.float32, 15), ("chi2", np.float32)])
 MERGED_DTYPE = np.dtype([("n_segments", np.int32), ("n_clusters", np.int32), ("segment_offset", np.int32), ("first_track", np.int32)])
-assert TRACK_DTYPE.itemsize == 112 and TRACKLET_DTYPE.itemsize == 116
+REFIT_DTYPE = np.dtype([("first_track", np.int32), ("sector", np.int32), ("n_fit", np.int32), ("ok", np.int32),
+                        ("x", np.float32), ("p", np.float32, 5), ("c", np.float32, 15), ("chi2", np.float32)])
+assert TRACK_DTYPE.itemsize == 112 and TRACKLET_DTYPE.itemsize == 116 and REFIT_DTYPE.itemsize == 104
 
 TPC_OK, TPC_E_ARG, TPC_E_STATE, TPC_E_NOMEM, TPC_E_OVERFLOW, TPC_E_CUDA = 0, -1, -2, -3, -4, -5
 TPC_DUMP_LINKS, TPC_DUMP_START_HITS, TPC_DUMP_TRACKLETS, TPC_DUMP_OWNERS = 1, 2, 3, 4
@@ -97,6 +100,8 @@ def lib():
         L.tpc_get_tracks.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(i32), ctypes.POINTER(vp), ctypes.POINTER(i64)]
         L.tpc_sync.argtypes = [vp]
         L.tpc_merge_tracks.argtypes = [vp]
+        L.tpc_refit_tracks.argtypes = [vp]
+        L.tpc_get_refit.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(i32)]
         L.tpc_get_merged.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(i32),
                                      ctypes.POINTER(vp), ctypes.POINTER(i32), ctypes.POINTER(vp)]
         L.tpc_get_stats.argtypes = [vp, ctypes.POINTER(tpc_stats)]
@@ -261,11 +266,23 @@ class Tracker:
         return {"next": arr(nx, n, np.int32), "prev": arr(pv, n, np.int32), "chi2": arr(ch, n, np.float32),
                 "merged": arr(mg, m, MERGED_DTYPE), "segments": arr(sg, n, np.int32)}
 
+    def refit_tracks(self):
+        return self._check(self._L.tpc_refit_tracks(self._h), "tpc_refit_tracks")
+
+    def get_refit(self):
+        """-> tpc_refit_track records, one per merged track (same order as get_merged()["merged"])."""
+        rp, n = ctypes.c_void_p(), ctypes.c_int32()
+        self._check(self._L.tpc_get_refit(self._h, ctypes.byref(rp), ctypes.byref(n)), "tpc_get_refit")
+        if not n.value:
+            return np.zeros(0, dtype=REFIT_DTYPE)
+        buf = (ctypes.c_char * (n.value * REFIT_DTYPE.itemsize)).from_address(rp.value)
+        return np.frombuffer(buf, dtype=REFIT_DTYPE).copy()
+
     def get_stats(self) -> dict:
         s = tpc_stats()
         self._check(self._L.tpc_get_stats(self._h, ctypes.byref(s)), "tpc_get_stats")
-        d = {k: int(getattr(s, k)) for k, _ in tpc_stats._fields_ if k not in ("kernel_us", "merge_us")}
-        d["merge_us"] = float(s.merge_us)
+        d = {k: int(getattr(s, k)) for k, _ in tpc_stats._fields_ if k not in ("kernel_us", "merge_us", "refit_us")}
+        d["merge_us"], d["refit_us"] = float(s.merge_us), float(s.refit_us)
         d["kernel_us"] = dict(zip(KERNEL_NAMES, [float(v) for v in s.kernel_us[:6]]))
         d["total_us"] = float(s.kernel_us[6])
         d["k6a_fused"] = bool(s.kernel_us[7] > 0.5)

@@ -104,6 +104,8 @@ struct DevPtrs {
                            // in each row, -1 none: indexes weight[] / orig[] directly
     tpc_track* tracks;
     uint32_t* clusterIds;
+    uint32_t* clusterPos;  // same order as clusterIds: global sorted position of the cluster (hits[] holds its y, z) ...
+    uint8_t* clusterRow;   // ... and its pad row: what the final fit (K8) reads
     uint32_t* counters;
     uint32_t* sectorGidBase;
     int32_t nRowsTotal;

@@ -251,4 +251,93 @@ __global__ void __launch_bounds__(kK7Threads) k7_chains(MergePtrs m) {
     }
 }
 
+// ------------------------------------------------------------------------------------------ K8
+// Final fit of the merged tracks (Phase II, second step, reading S8): ONE inward Kalman pass over all
+// clusters of a merged track, outermost cluster first (it is the starting point), across the sector frames of its
+// segments (k7_rotate); per step the curvature constant follows the field polynomial at the state's point and the
+// multiple scattering over the step's path is added to the covariance.  One thread per merged track: the pass is a
+// chain of up to ~450 dependent steps, so what bounds the kernel is that chain for the longest merged track.
+__device__ __forceinline__ float k8_field_cb(const KFState& a, float x, float CB, float ar, float az) {
+    const float r2 = x * x + a.p0 * a.p0;
+    return CB * (1.0f + ar * r2 + az * (a.p1 * a.p1));
+}
+__device__ __forceinline__ void k8_scatter(KFState& a, float L, float x0inv) {
+    const float s = a.p2, t = a.p3, k = a.p4;
+    const float one_t2 = 1.0f + t * t;
+    const float th2 = (0.0136f * 0.0136f) * ((k * k) / one_t2) * (L * x0inv);
+    a.c5 = a.c5 + (th2 * (1.0f - s * s)) * one_t2;
+    a.c9 = a.c9 + (th2 * one_t2) * one_t2;
+    a.c13 = a.c13 + ((th2 * t) * k) * one_t2;
+    a.c14 = a.c14 + ((th2 * t) * t) * (k * k);
+}
+
+__global__ void __launch_bounds__(kK7Threads) k8_refit(MergePtrs m, DevPtrs d, DevParams dp, tpc_refit_track* __restrict__ out,
+                                                       int perSide, float cosB, float sinB) {
+    const unsigned nM = m.mcount[0];
+    const tpc_params& P = dp.P;
+    for (unsigned i = blockIdx.x * kK7Threads + threadIdx.x; i < nM; i += gridDim.x * kK7Threads) {
+        const tpc_merged_track M = m.merged[i];
+        const int32_t* segs = m.segments + M.segment_offset;
+        const tpc_track inner = m.tracks[segs[0]];
+        const tpc_track outer = m.tracks[segs[M.n_segments - 1]];
+        KFState st;
+        st.p0 = outer.p[0]; st.p1 = outer.p[1]; st.p2 = outer.p[2]; st.p3 = outer.p[3]; st.p4 = outer.p[4];
+        st.c0 = st.c1 = st.c2 = st.c3 = st.c4 = st.c5 = st.c6 = st.c7 = st.c8 = st.c9 = st.c10 = st.c11 = st.c12 = st.c13 = st.c14 = 0.f;
+        float x = outer.x, chi2 = 0.f;
+        int nfit = 0, curSector = outer.sector;
+        KFState nw;
+        bool ok = kf_propagate(st, d.rowX[outer.last_row] - x, k8_field_cb(st, x, dp.CB, P.field_ar, P.field_az), P.kf_smax, nw);
+        if (ok) st = nw;
+        bool first = true;
+        for (int sg = M.n_segments - 1; ok && sg >= 0; sg--) {
+            const tpc_track seg = m.tracks[segs[sg]];
+            for (int c = seg.n_clusters - 1; ok && c >= 0; c--) {
+                const unsigned at = (unsigned)seg.cluster_offset + (unsigned)c;
+                const float2 h = d.hits[d.clusterPos[at]];
+                const float xr = d.rowX[d.clusterRow[at]];
+                if (first) {           // the outermost cluster is the starting point, not a measurement
+                    st.p0 = h.x; st.p1 = h.y; x = xr;
+                    kf_init_cov(st, P);
+                    chi2 = 0.f; nfit = 0;
+                    first = false;
+                    continue;
+                }
+                if (seg.sector != curSector) {       // into the next segment's sector frame
+                    int dsec = seg.sector % perSide - curSector % perSide;
+                    if (dsec > perSide / 2) dsec -= perSide;
+                    if (dsec < -perSide / 2) dsec += perSide;
+                    ok = k7_rotate(st, x, cosB, dsec > 0 ? sinB : -sinB, k8_field_cb(st, x, dp.CB, P.field_ar, P.field_az), P.kf_smax);
+                    curSector = seg.sector;
+                    if (!ok) break;
+                }
+                const float x0 = x, y0 = st.p0, z0 = st.p1;
+                ok = kf_propagate(st, xr - x, k8_field_cb(st, x, dp.CB, P.field_ar, P.field_az), P.kf_smax, nw);
+                if (!ok) break;
+                st = nw; x = xr;
+                if (P.ms_x0_inv > 0.f) {
+                    const float dx = x - x0, dy = st.p0 - y0, dz = st.p1 - z0;
+                    k8_scatter(st, sqrtf((dx * dx + dy * dy) + dz * dz), P.ms_x0_inv);
+                }
+                kf_update_hit(st, h.x, h.y, P.err2_y, P.err2_z, chi2, true);
+                nfit++;
+            }
+        }
+        tpc_refit_track r;
+        r.first_track = segs[0];
+        if (ok && !first) {
+            r.sector = curSector; r.n_fit = nfit; r.ok = 1; r.x = x; r.chi2 = chi2;
+            r.p[0] = st.p0; r.p[1] = st.p1; r.p[2] = st.p2; r.p[3] = st.p3; r.p[4] = st.p4;
+            r.c[0] = st.c0; r.c[1] = st.c1; r.c[2] = st.c2; r.c[3] = st.c3; r.c[4] = st.c4; r.c[5] = st.c5; r.c[6] = st.c6; r.c[7] = st.c7;
+            r.c[8] = st.c8; r.c[9] = st.c9; r.c[10] = st.c10; r.c[11] = st.c11; r.c[12] = st.c12; r.c[13] = st.c13; r.c[14] = st.c14;
+        } else {                       // the pass could not be completed: the innermost segment's Phase-I state
+            r.sector = inner.sector; r.n_fit = 0; r.ok = 0; r.x = inner.x; r.chi2 = inner.chi2;
+#pragma unroll
+            for (int q = 0; q < 5; q++) r.p[q] = inner.p[q];
+#pragma unroll
+            for (int q = 0; q < 15; q++) r.c[q] = inner.c[q];
+        }
+        out[i] = r;
+    }
+}
+
 }  // namespace tpc

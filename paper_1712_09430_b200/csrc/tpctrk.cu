@@ -24,7 +24,7 @@ inline size_t align_up(size_t v, size_t a = kAlign) { return (v + a - 1) / a * a
 
 struct Layout {   // byte offsets into the workspace
     size_t inY, inZ, grid, meta, rowX, hits, orig, binStart, buckets, linkUp, linkDn, linkUpC, linkDnC, weight, starts, startsRaw, rowHist, rowStartBase, recs, rowHit,
-        tracks, clusterIds, counters, sectorGidBase,
+        tracks, clusterIds, clusterPos, clusterRow, refit, counters, sectorGidBase,
         mKey, mBinStart, mBinCursor, mOrder, mBestIn, mOut, mOutChi2, mNext, mPrev, mChi2, mMerged, mSegments, mCount, total;
     int64_t hitCap, binCap, maxTracklets;
     enum : int { kMaxGuards = 64 };
@@ -72,7 +72,13 @@ struct tpc_tracker {
     cudaEvent_t evM0 = nullptr, evM1 = nullptr;
     int32_t* outNext = nullptr; int32_t* outPrev = nullptr; float* outMChi2 = nullptr; tpc_merged_track* outMerged = nullptr;
     int32_t* outSegments = nullptr; uint32_t* outMCount = nullptr; int64_t outMergeCap = 0;
-    float mergeUs = 0.f; int32_t nMerged = 0, nMergeLinks = 0;                   // how often the estimate was short (tpc_stats)
+    float mergeUs = 0.f; int32_t nMerged = 0, nMergeLinks = 0;
+    // Phase II final fit
+    tpc_refit_track* devRefit = nullptr;
+    bool refitted = false, refitFetched = false;
+    cudaEvent_t evR0 = nullptr, evR1 = nullptr;
+    tpc_refit_track* outRefit = nullptr; int64_t outRefitCap = 0;
+    float refitUs = 0.f;                   // how often the estimate was short (tpc_stats)
     RowGrid* hostGrid = nullptr;            // pinned
     RowMeta* hostMeta = nullptr;            // pinned
     uint32_t* hostSectorBase = nullptr;     // pinned
@@ -140,6 +146,9 @@ Layout make_layout(const tpc_tracker* t, int64_t maxClusters) {
     L.rowHit = take(sizeof(int32_t) * L.maxTracklets * t->rhStride);
     L.tracks = take(sizeof(tpc_track) * L.maxTracklets);
     L.clusterIds = take(sizeof(uint32_t) * (maxClusters + 16));
+    L.clusterPos = take(sizeof(uint32_t) * (maxClusters + 16));
+    L.clusterRow = take(sizeof(uint8_t) * (maxClusters + 16));
+    L.refit = take(sizeof(tpc_refit_track) * L.maxTracklets);
     L.counters = take(sizeof(uint32_t) * (kNCounters + kMaxPending));
     L.sectorGidBase = take(sizeof(uint32_t) * (t->nSec + 1));
     // K7 (Phase II merging): per-track words, sized like the track output
@@ -176,6 +185,7 @@ void bind_pointers(tpc_tracker* t) {
     d.weight = (uint32_t*)(w + L.weight); d.starts = (int4*)(w + L.starts); d.startsRaw = (int4*)(w + L.startsRaw); d.rowHist = (uint32_t*)(w + L.rowHist); d.rowStartBase = (const uint32_t*)(w + L.rowStartBase);
     d.recs = (TrackletRec*)(w + L.recs); d.rowHit = (int32_t*)(w + L.rowHit);
     d.tracks = (tpc_track*)(w + L.tracks); d.clusterIds = (uint32_t*)(w + L.clusterIds);
+    d.clusterPos = (uint32_t*)(w + L.clusterPos); d.clusterRow = (uint8_t*)(w + L.clusterRow);
     d.counters = (uint32_t*)(w + L.counters); d.sectorGidBase = (uint32_t*)(w + L.sectorGidBase);
     d.nRowsTotal = t->nRowsTotal; d.maxTracklets = (int32_t)std::min<int64_t>(L.maxTracklets, 0x7fffffff);
     d.rhStride = t->rhStride;
@@ -186,6 +196,7 @@ void bind_pointers(tpc_tracker* t) {
     m.outChi2 = (float*)(w + L.mOutChi2); m.next = (int32_t*)(w + L.mNext); m.prev = (int32_t*)(w + L.mPrev);
     m.chi2 = (float*)(w + L.mChi2); m.merged = (tpc_merged_track*)(w + L.mMerged); m.segments = (int32_t*)(w + L.mSegments);
     m.mcount = (uint32_t*)(w + L.mCount); m.nBins = t->nRowsTotal;
+    t->devRefit = (tpc_refit_track*)(w + L.refit);
 }
 
 // Page-locked host memory (cudaMallocHost / cudaHostRegister, e.g. a pinned torch tensor): the DMA engine can read it
@@ -440,6 +451,7 @@ void tpc_default_params(tpc_params* p) {
     p->road_nsig = 4.0f; p->road_max = 2.0f;
     p->max_gap = 4; p->min_hits = 10; p->seed_min_chain = 3;
     p->merge_chi2 = 50.0f; p->merge_max_row_gap = 40;
+    p->field_ar = 0.0f; p->field_az = 0.0f; p->ms_x0_inv = 0.0f;
     p->max_tracklets_per_cluster = 0.1f;
     p->grid_bins_per_hit = 2.0f;
 }
@@ -466,7 +478,8 @@ int tpc_tracker_create(const tpc_geometry* g, float bz_tesla, tpc_tracker** out)
                         pos(P.road_nsig) && pos(P.road_max) && P.kf_smax > 0.f && P.kf_smax < 1.f &&
                         nonneg(P.nf_ty) && nonneg(P.nf_tz) && nonneg(P.nf_c) && nonneg(P.nf_d2max) &&
                         P.seed_min_chain >= 2 && P.min_hits >= 1 && P.max_gap >= 0 && pos(P.max_tracklets_per_cluster) &&
-                        P.grid_bins_per_hit >= 0.25f && P.grid_bins_per_hit <= 64.f && nonneg(P.merge_chi2) && P.merge_max_row_gap >= 0 && bz_tesla == bz_tesla && std::abs(bz_tesla) < 1e3f;
+                        P.grid_bins_per_hit >= 0.25f && P.grid_bins_per_hit <= 64.f && nonneg(P.merge_chi2) && P.merge_max_row_gap >= 0 &&
+                        nonneg(P.ms_x0_inv) && std::abs(P.field_ar) < 1e30f && std::abs(P.field_az) < 1e30f && bz_tesla == bz_tesla && std::abs(bz_tesla) < 1e3f;
         if (!ok) { delete t; return TPC_E_ARG; }
     }
     t->sectorDphi = g->sector_dphi;
@@ -495,6 +508,9 @@ void tpc_tracker_destroy(tpc_tracker* t) {
     if (t->evDone) cudaEventDestroy(t->evDone);
     if (t->evM0) cudaEventDestroy(t->evM0);
     if (t->evM1) cudaEventDestroy(t->evM1);
+    if (t->evR0) cudaEventDestroy(t->evR0);
+    if (t->evR1) cudaEventDestroy(t->evR1);
+    if (t->outRefit) cudaFreeHost(t->outRefit);
     for (void* q : {(void*)t->outNext, (void*)t->outPrev, (void*)t->outMChi2, (void*)t->outMerged, (void*)t->outSegments, (void*)t->outMCount})
         if (q) cudaFreeHost(q);
     delete t;
@@ -700,7 +716,7 @@ int tpc_track_sectors(tpc_tracker* t) {
     // tpc_get_tracks waits once and normally copies nothing.
     rc = queue_download(t);
     if (rc != TPC_OK) return rc;
-    t->tracked = true; t->fetched = false; t->merged = false; t->mergeFetched = false;
+    t->tracked = true; t->fetched = false; t->merged = false; t->mergeFetched = false; t->refitted = false; t->refitFetched = false;
     return TPC_OK;
 }
 
@@ -724,7 +740,47 @@ int tpc_merge_tracks(tpc_tracker* t) {
     k7_chains<<<grid, kK7Threads, 0, s>>>(m);
     CUDA_TRY(t, cudaEventRecord(t->evM1, s));
     CUDA_TRY(t, cudaGetLastError());
-    t->merged = true; t->mergeFetched = false;
+    t->merged = true; t->mergeFetched = false; t->refitted = false; t->refitFetched = false;
+    return TPC_OK;
+}
+
+int tpc_refit_tracks(tpc_tracker* t) {
+    if (!t) return TPC_E_ARG;
+    if (!t->merged) return TPC_E_STATE;
+    cudaStream_t s = t->stream;
+    if (!t->evR0) { CUDA_TRY(t, cudaEventCreate(&t->evR0)); CUDA_TRY(t, cudaEventCreate(&t->evR1)); }
+    DevParams dp; dp.P = t->P; dp.CB = t->CB; dp.nSec = t->nSec; dp.nRows = t->nRows;
+    const int perSide = t->nSec >= 36 ? 18 : t->nSec;
+    const float cosB = (float)std::cos((double)t->sectorDphi), sinB = (float)std::sin((double)t->sectorDphi);
+    CUDA_TRY(t, cudaEventRecord(t->evR0, s));
+    k8_refit<<<t->k6Blocks, kK7Threads, 0, s>>>(t->mp, t->dev, dp, t->devRefit, perSide, cosB, sinB);
+    CUDA_TRY(t, cudaEventRecord(t->evR1, s));
+    CUDA_TRY(t, cudaGetLastError());
+    t->refitted = true; t->refitFetched = false;
+    return TPC_OK;
+}
+
+int tpc_get_refit(tpc_tracker* t, const tpc_refit_track** refit, int32_t* n_merged) {
+    if (!t) return TPC_E_ARG;
+    if (!t->refitted) return TPC_E_STATE;
+    int rc = tpc_get_merged(t, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr);     // the counts
+    if (rc != TPC_OK) return rc;
+    const int64_t nM = t->nMerged;
+    if (!t->refitFetched) {
+        if (nM + 1 > t->outRefitCap) {
+            if (t->outRefit) cudaFreeHost(t->outRefit);
+            t->outRefitCap = std::max<int64_t>(nM + 1, 1024) * 3 / 2;
+            CUDA_TRY(t, cudaMallocHost(&t->outRefit, sizeof(tpc_refit_track) * t->outRefitCap));
+        }
+        if (nM) CUDA_TRY(t, cudaMemcpyAsync(t->outRefit, t->devRefit, sizeof(tpc_refit_track) * nM, cudaMemcpyDeviceToHost, t->stream));
+        CUDA_TRY(t, cudaStreamSynchronize(t->stream));
+        float ms = 0.f;
+        CUDA_TRY(t, cudaEventElapsedTime(&ms, t->evR0, t->evR1));
+        t->refitUs = ms * 1000.f;
+        t->refitFetched = true;
+    }
+    if (refit) *refit = t->outRefit;
+    if (n_merged) *n_merged = (int32_t)nM;
     return TPC_OK;
 }
 
@@ -829,6 +885,7 @@ int tpc_get_stats(tpc_tracker* t, tpc_stats* out) {
     out->max_tracklets = t->ws ? t->dev.maxTracklets : 0;
     out->workspace_bytes_used = (int64_t)t->L.total;
     out->n_output_refetches = t->nRefetch;
+    if (t->refitFetched) out->refit_us = t->refitUs;
     if (t->mergeFetched) { out->merge_us = t->mergeUs; out->n_merged_tracks = t->nMerged; out->n_merge_links = t->nMergeLinks; }
     if (!t->tracked) return TPC_OK;
     out->n_links = t->counters[kNLinks];

@@ -27,7 +27,7 @@ def test_library_exports_every_declared_symbol():
 
 
 def test_struct_layouts_match_header():
-    assert ctypes.sizeof(binding.tpc_params) == 19 * 4
+    assert ctypes.sizeof(binding.tpc_params) == 22 * 4
     assert ctypes.sizeof(binding.tpc_stats) == 11 * 8 + 4 * 4 + 8 * 4
     assert binding.TRACK_DTYPE.itemsize == 112
     p = binding.default_params()

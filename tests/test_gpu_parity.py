@@ -742,3 +742,74 @@ def test_track_merging_hand_made_cases_and_parameters():
     trk.merge_tracks()
     g = trk.get_merged()
     assert g["next"].size == 0 and g["merged"].size == 0
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Phase II, second step: final fit of the merged tracks (K8) against the oracle's S8
+
+def _compare_refit(trk, tracks, ids, ref, rtol=1e-4, atol=1e-5):
+    g = trk.get_merged()
+    rf = trk.get_refit()
+    assert rf.size == g["merged"].size and np.array_equal(rf["first_track"], g["merged"]["first_track"])
+    key_g = ids[tracks["cluster_offset"]].astype(np.int64)
+    key_o = ref.cluster_ids[ref.tracks["cluster_offset"]].astype(np.int64)
+    # merged tracks keyed by the first cluster of their innermost segment
+    kg = key_g[rf["first_track"]]
+    ko = key_o[ref.refits["first_track"]]
+    assert np.array_equal(np.sort(kg), np.sort(ko))
+    a, b = rf[np.argsort(kg)], ref.refits[np.argsort(ko)]
+    for f in ("sector", "n_fit", "ok"):
+        assert np.array_equal(a[f], b[f]), f
+    out = {"n_merged": int(rf.size), "n_ok": int(a["ok"].sum())}
+    for f in ("x", "p", "c", "chi2"):
+        x, y = a[f].astype(np.float64), b[f]
+        assert np.all(np.abs(x - y) <= atol + rtol * np.abs(y)), (f, np.abs(x - y).max())
+        out[f"bitexact_{f}"] = bool(np.array_equal(x.astype(np.float32), y.astype(np.float32)))
+    assert trk.debug_check_guards() == 0
+    return out
+
+
+@pytest.mark.parametrize("cfg,seed,field,ms", [(1, 0, 0.0, 0.0), (2, 0, 0.0, 0.0), (2, 4, -2e-6, 1.0 / 3000.0), (3, 0, 0.0, 0.0)])
+def test_final_fit_matches_the_oracle(cfg, seed, field, ms, capsys):
+    """tpc_refit_tracks (K8) on the merged tracks of configs 1-3, with the constant field and without process noise
+    (the generator's world) and with a field polynomial and multiple scattering switched on: every record (frame,
+    number of clusters used, state, covariance, chi2) equals the oracle's S8 within 1e-4 rel / 1e-5 abs."""
+    _cuda()
+    ev = datagen.config_event(cfg, seed=seed)
+    po, pg = _merge_oracle_params(), binding.default_params()
+    po.field_ar = pg.field_ar = field
+    po.field_az = pg.field_az = field / 2
+    po.ms_x0_inv = pg.ms_x0_inv = ms
+    po.field_ar, po.field_az, po.ms_x0_inv = float(np.float32(field)), float(np.float32(field / 2)), float(np.float32(ms))
+    o = oracle.Oracle(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz, po)
+    ref = o.refit(o.merge(o.run(ev.row_counts, ev.y, ev.z)))
+    trk, tracks, ids = run_gpu(ev, pg)
+    trk.merge_tracks()
+    trk.refit_tracks()
+    out = _compare_refit(trk, tracks, ids, ref)
+    assert out["n_ok"] >= 0.95 * out["n_merged"]
+    st = trk.get_stats()
+    with capsys.disabled():
+        print(f"\n[refit config {cfg} seed {seed} field {field} ms {ms}] {out} K8 {st['refit_us']:.1f} us")
+
+
+def test_final_fit_call_order_and_empty_event():
+    torch = _cuda()
+    ev = datagen.config_event(1, seed=2)
+    trk, tracks, ids = run_gpu(ev)
+    with pytest.raises(binding.TpcError) as e:
+        trk.refit_tracks()                              # before tpc_merge_tracks
+    assert e.value.code == binding.TPC_E_STATE
+    trk.merge_tracks()
+    with pytest.raises(binding.TpcError) as e:
+        trk.get_refit()                                 # before tpc_refit_tracks
+    assert e.value.code == binding.TPC_E_STATE
+    trk.refit_tracks()
+    a = trk.get_refit()
+    trk.refit_tracks()
+    b = trk.get_refit()
+    assert a.size > 0 and a.tobytes() == b.tobytes()
+    empty = datagen.event_from_hits([], 36, datagen.default_row_x(), 0.5)
+    trk, tracks, ids = run_gpu(empty, max_clusters=16)
+    trk.merge_tracks(); trk.refit_tracks()
+    assert trk.get_refit().size == 0
