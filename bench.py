@@ -452,18 +452,23 @@ def main():
     st = trk.get_stats()
     value, ms, n_total = aggregate(dist, dev, ev.n_clusters, step_ms)
 
-    # ---- Phase II track merging (K7; extra key, not part of the metric): device time of
-    # tpc_merge_tracks on the tracks of this event, L2 flushed before, CUDA events inside the library
-    merge_us = []
+    # ---- Phase II: track merging (K7) and final fit (K8, next-2); extra key, not part of the
+    # metric: device times of tpc_merge_tracks / tpc_refit_tracks on the tracks of this event, L2 flushed before, CUDA events inside the library
+    merge_us, refit_us = [], []
     for _ in range(max(3, min(args.steps, 10))):
         flush.fill_(1)
         trk.track_sectors()
         trk.merge_tracks()
+        trk.refit_tracks()
         trk.get_merged()
+        trk.get_refit()
         merge_us.append(trk.get_stats()["merge_us"])
+        refit_us.append(trk.get_stats()["refit_us"])
     stm = trk.get_stats()
     merge_leg = {"kernel": "K7 track merging (tpc_merge_tracks: 7 launches)", "us": round(sum(merge_us[1:]) / len(merge_us[1:]), 1),
-                 "n_tracks": stm["n_tracks"], "n_links": stm["n_merge_links"], "n_merged_tracks": stm["n_merged_tracks"]}
+                 "n_tracks": stm["n_tracks"], "n_links": stm["n_merge_links"], "n_merged_tracks": stm["n_merged_tracks"],
+                 "refit_kernel": "K8 final fit of the merged tracks (tpc_refit_tracks: 1 launch)",
+                 "refit_us": round(sum(refit_us[1:]) / len(refit_us[1:]), 1)}
 
     # ---- end to end through the C ABI with HOST buffers (pinned), H2D + D2H of every step inside the timed region.
     # ONE host thread keeps n_pipe tracker instances (each on its own stream) in flight, round robin: for the oldest
