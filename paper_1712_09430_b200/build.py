@@ -9,7 +9,7 @@ _ROOT = os.path.dirname(_PKG)
 CSRC = os.path.join(_PKG, "csrc")
 LIB = os.path.join(_PKG, "libtpctrk.so")
 SOURCES = [os.path.join(CSRC, "tpctrk.cu")]
-HEADERS = [os.path.join(CSRC, f) for f in ("device_types.cuh", "kernels_ca.cuh", "kernels_kf.cuh")] + [
+HEADERS = [os.path.join(CSRC, f) for f in ("device_types.cuh", "kernels_ca.cuh", "kernels_kf.cuh", "kernels_merge.cuh")] + [
     os.path.join(_ROOT, "include", "tpctrk.h")]
 
 # -fmad=false: no FMA contraction, so every fp32 decision value equals the written IEEE expression
