@@ -40,7 +40,8 @@ typedef enum tpc_error {
     TPC_E_NOMEM = -3,    /* workspace too small for the loaded clusters; see tpc_workspace_bytes */
     TPC_E_OVERFLOW = -4, /* tracklet-capacity estimate exceeded ("estimation was too small");
                             tpc_stats.n_start_hits holds the required capacity; enlarge and re-run */
-    TPC_E_CUDA = -5      /* CUDA runtime error or no device; tpc_last_cuda_error() has the code */
+    TPC_E_CUDA = -5,     /* CUDA runtime error or no device; tpc_last_cuda_error() has the code */
+    TPC_E_LIMIT = -6     /* tpc_merge_links_no_alloc: more tracks or (sector,row) bins than its fixed scratch holds */
 } tpc_error;
 
 /* Constants of the method (the paper gives none). */
@@ -249,6 +250,37 @@ typedef struct tpc_refit_track {
 int tpc_refit_tracks(tpc_tracker* t);
 /* Synchronise and download: refit[i] belongs to merged[i] of tpc_get_merged (same event).  Library-owned pinned memory. */
 int tpc_get_refit(tpc_tracker* t, const tpc_refit_track** refit, int32_t* n_merged);
+
+/* ---- Track merging without any allocation (for callers that cannot call cudaMalloc: code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid it) ----
+ * The K7 kernels of tpc_merge_tracks (same reading S7, same arithmetic, same links and chi2) with their scratch - the
+ * tracks' keys, the (sector, first row) bin table, the ordered track list, the best-partner words, the counters - in
+ * ONE file-scope `static __device__` array of the library instead of a tracker workspace: no tracker, no workspace,
+ * and neither this call nor anything it calls uses cudaMalloc, cudaFree, cudaMallocHost or an allocating library
+ * routine.  The array is sized for TPC_NO_ALLOC_MAX_TRACKS tracks and TPC_NO_ALLOC_MAX_BINS = n_sectors * n_rows bins
+ * (about 1.7 MB); every GPU on which the library's kernels are loaded holds it until the process exits.
+ *
+ * Inputs (caller-owned DEVICE memory of the current device): dev_tracks[n_tracks] as tpc_get_tracks returns them
+ * (sector < n_sectors, first_row <= last_row < n_rows, cluster_offset into dev_cluster_ids), dev_cluster_ids = the
+ * cluster-id array of the same event (only the first id of each track is read: it is the track's canonical key).
+ * Outputs (caller-owned DEVICE memory, n_tracks entries each): dev_next / dev_prev / dev_chi2 as tpc_get_merged's
+ * next / prev / chi2.  params: host pointer or NULL = defaults; kf_smax, merge_chi2 and merge_max_row_gap are used.
+ * Asynchronous on cuda_stream (a cudaStream_t of the current device, NULL = default stream): the outputs are valid
+ * once the stream has reached the end of the call's work.
+ *
+ * The scratch is shared by every call on the same device and keeps the last call's contents; each call clears what
+ * must start clean (bin counts, cursors, best-partner words, counters) on the stream before it uses it.  Calls whose
+ * GPU work overlaps on one device - two streams, two host threads - RACE on the scratch: serialise them (one stream,
+ * or an event between them).  The first call on a device looks the array's address up (cudaGetSymbolAddress, once
+ * per device, under a lock).
+ * Errors: TPC_E_ARG (null pointer with n_tracks > 0, n_tracks < 0, geometry or parameters out of their domain),
+ * TPC_E_LIMIT (n_tracks > TPC_NO_ALLOC_MAX_TRACKS or n_sectors * n_rows > TPC_NO_ALLOC_MAX_BINS: nothing is launched;
+ * use tpc_merge_tracks with a workspace instead), TPC_E_CUDA (*cuda_error, if not NULL, receives the cudaError_t). */
+#define TPC_NO_ALLOC_MAX_TRACKS 65536
+#define TPC_NO_ALLOC_MAX_BINS 16384
+int tpc_merge_links_no_alloc(int32_t n_sectors, int32_t n_rows, float sector_dphi, float bz_tesla, const tpc_params* params,
+                             const tpc_track* dev_tracks, int32_t n_tracks, const uint32_t* dev_cluster_ids,
+                             int32_t* dev_next, int32_t* dev_prev, float* dev_chi2, void* cuda_stream, int* cuda_error);
 
 /* Stage parity hooks (tests): copy one stage's buffers, converted to canonical (load-index) form, to host_dst.
  * Synchronous; allocates temporary device memory.  bytes must equal tpc_debug_dump_bytes(t, stage). */

@@ -59,7 +59,8 @@ REFIT_DTYPE = np.dtype([("first_track", np.int32), ("sector", np.int32), ("n_fit
                         ("x", np.float32), ("p", np.float32, 5), ("c", np.float32, 15), ("chi2", np.float32)])
 assert TRACK_DTYPE.itemsize == 112 and TRACKLET_DTYPE.itemsize == 116 and REFIT_DTYPE.itemsize == 104
 
-TPC_OK, TPC_E_ARG, TPC_E_STATE, TPC_E_NOMEM, TPC_E_OVERFLOW, TPC_E_CUDA = 0, -1, -2, -3, -4, -5
+TPC_OK, TPC_E_ARG, TPC_E_STATE, TPC_E_NOMEM, TPC_E_OVERFLOW, TPC_E_CUDA, TPC_E_LIMIT = 0, -1, -2, -3, -4, -5, -6
+TPC_NO_ALLOC_MAX_TRACKS, TPC_NO_ALLOC_MAX_BINS = 65536, 16384
 TPC_DUMP_LINKS, TPC_DUMP_START_HITS, TPC_DUMP_TRACKLETS, TPC_DUMP_OWNERS = 1, 2, 3, 4
 KERNEL_NAMES = ("K1_sort_grid", "K2_neighbours", "K3K4_clean_start", "K5_construct", "K6a_weights", "K6b_select")
 
@@ -113,6 +114,8 @@ def lib():
         L.tpc_strerror.restype = ctypes.c_char_p
         L.tpc_last_cuda_error.argtypes = [vp]
         L.tpc_launches_per_track.argtypes = [vp]
+        L.tpc_merge_links_no_alloc.argtypes = [i32, i32, ctypes.c_float, ctypes.c_float, ctypes.POINTER(tpc_params), vp, i32, vp,
+                                               vp, vp, vp, vp, ctypes.POINTER(ctypes.c_int)]
         _lib = L
     return _lib
 
@@ -128,6 +131,20 @@ def default_params() -> tpc_params:
     p = tpc_params()
     lib().tpc_default_params(ctypes.byref(p))
     return p
+
+
+def merge_links_no_alloc(n_sectors, n_rows, sector_dphi, bz_tesla, params, dev_tracks, n_tracks, dev_cluster_ids,
+                         dev_next, dev_prev, dev_chi2, stream=None):
+    """tpc_merge_links_no_alloc: K7's links for caller-owned DEVICE arrays (torch tensors or raw device pointers), its
+    scratch in the library's static device array; allocates nothing.  Asynchronous on `stream` (a cudaStream_t as int)."""
+    err = ctypes.c_int(0)
+    dp = lambda a: a if isinstance(a, (int, type(None))) else a.data_ptr()
+    rc = lib().tpc_merge_links_no_alloc(int(n_sectors), int(n_rows), float(sector_dphi), float(bz_tesla),
+                                        ctypes.byref(params) if params is not None else None, dp(dev_tracks), int(n_tracks),
+                                        dp(dev_cluster_ids), dp(dev_next), dp(dev_prev), dp(dev_chi2),
+                                        int(stream) if stream else None, ctypes.byref(err))
+    if rc != TPC_OK:
+        raise TpcError(rc, "tpc_merge_links_no_alloc", err.value)
 
 
 def _ptr(a):

@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -978,6 +979,7 @@ const char* tpc_strerror(int code) {
         case TPC_E_NOMEM: return "workspace too small";
         case TPC_E_OVERFLOW: return "tracklet capacity exceeded";
         case TPC_E_CUDA: return "CUDA error or no device";
+        case TPC_E_LIMIT: return "more tracks or (sector,row) bins than the fixed scratch of tpc_merge_links_no_alloc holds";
         default: return "unknown error";
     }
 }
@@ -985,3 +987,112 @@ const char* tpc_strerror(int code) {
 int tpc_last_cuda_error(const tpc_tracker* t) { return t ? t->lastCuda : 0; }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------------------------------ K7 without allocation
+// tpc_merge_links_no_alloc (tpctrk.h): the K7 kernels of tpc_merge_tracks on caller-owned tracks and outputs, their
+// scratch in the file-scope array below instead of a tracker workspace.  Nothing here allocates.
+namespace {
+
+constexpr size_t kNaMaxT = TPC_NO_ALLOC_MAX_TRACKS, kNaMaxB = TPC_NO_ALLOC_MAX_BINS;
+constexpr size_t na_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
+// sections of the scratch array [bytes from its start], each a multiple of 256
+constexpr size_t kNaCounters = 0;                                              // uint32[kNCounters]: [kNTracks] = n_tracks
+constexpr size_t kNaMCount = kNaCounters + na_up(sizeof(uint32_t) * kNCounters);   // uint32[2] (k7_init clears it)
+constexpr size_t kNaKey = kNaMCount + kAlign;                                  // uint32[maxT]
+constexpr size_t kNaOrder = kNaKey + na_up(sizeof(uint32_t) * kNaMaxT);     // uint32[maxT]
+constexpr size_t kNaBestIn = kNaOrder + na_up(sizeof(uint32_t) * kNaMaxT);  // uint64[maxT]
+constexpr size_t kNaOut = kNaBestIn + na_up(sizeof(unsigned long long) * kNaMaxT);   // int32[maxT]
+constexpr size_t kNaOutChi2 = kNaOut + na_up(sizeof(int32_t) * kNaMaxT);    // float[maxT]
+constexpr size_t kNaBinStart = kNaOutChi2 + na_up(sizeof(float) * kNaMaxT); // uint32[maxB + 2]
+constexpr size_t kNaBinCursor = kNaBinStart + na_up(sizeof(uint32_t) * (kNaMaxB + 2));   // uint32[maxB + 1]
+constexpr size_t kNaBytes = kNaBinCursor + na_up(sizeof(uint32_t) * (kNaMaxB + 1));
+static_assert(kNaBytes < (2u << 20), "the no-allocation scratch is meant to stay modest (tpctrk.h says about 1.7 MB)");
+
+}  // namespace
+
+// In host code this name is a stand-in for the symbol, not a device address: kernels get the pointer that
+// cudaGetSymbolAddress returns for the current device (na_device below); device code may name the array directly.
+static __device__ __align__(256) unsigned char g_k7NaScratch[kNaBytes];
+
+namespace {
+
+// the track count where the K7 kernels look for it, the other counters zero (device code: names the array itself)
+__global__ void k7na_begin(int nTracks) {
+    uint32_t* c = reinterpret_cast<uint32_t*>(g_k7NaScratch + kNaCounters);
+    if (threadIdx.x < kNCounters) c[threadIdx.x] = threadIdx.x == kNTracks ? (uint32_t)nTracks : 0u;
+}
+
+struct NaDevice { unsigned char* scratch = nullptr; int blocks = 0; };
+constexpr int kNaMaxDevices = 64;
+NaDevice g_naDev[kNaMaxDevices];
+std::mutex g_naLock;
+
+// Once per device, with that device current: the device address of the scratch array and the grid of the K7 kernels.
+cudaError_t na_device(int dev, NaDevice& out) {
+    std::lock_guard<std::mutex> lk(g_naLock);
+    NaDevice& d = g_naDev[dev];
+    if (!d.scratch) {
+        void* p = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&p, g_k7NaScratch);
+        if (e != cudaSuccess) return e;
+        int sms = 0, occ = 0;
+        if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+        if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k7_match, kK7Threads, 0)) != cudaSuccess) return e;
+        d.blocks = std::max(1, sms) * std::max(1, occ);
+        d.scratch = static_cast<unsigned char*>(p);
+    }
+    out = d;
+    return cudaSuccess;
+}
+
+}  // namespace
+
+extern "C" int tpc_merge_links_no_alloc(int32_t n_sectors, int32_t n_rows, float sector_dphi, float bz_tesla, const tpc_params* params,
+                                        const tpc_track* dev_tracks, int32_t n_tracks, const uint32_t* dev_cluster_ids,
+                                        int32_t* dev_next, int32_t* dev_prev, float* dev_chi2, void* cuda_stream, int* cuda_error) {
+    if (cuda_error) *cuda_error = 0;
+    auto cuda_fail = [&](cudaError_t e) { if (cuda_error) *cuda_error = (int)e; return (int)TPC_E_CUDA; };
+    if (n_sectors < 1 || n_rows < 3 || n_rows > kMaxRows || n_tracks < 0) return TPC_E_ARG;
+    if ((int64_t)n_sectors * n_rows > (int64_t)kNaMaxB || (int64_t)n_tracks > (int64_t)kNaMaxT) return TPC_E_LIMIT;
+    if (n_tracks > 0 && (!dev_tracks || !dev_cluster_ids || !dev_next || !dev_prev || !dev_chi2)) return TPC_E_ARG;
+    tpc_params P;
+    if (params) P = *params; else tpc_default_params(&P);
+    if (!(P.kf_smax > 0.f && P.kf_smax < 1.f) || !(P.merge_chi2 >= 0.f && P.merge_chi2 < 1e30f) || P.merge_max_row_gap < 0 ||
+        !(std::abs(bz_tesla) < 1e3f) || !(std::abs(sector_dphi) < 1e3f)) return TPC_E_ARG;
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e);
+    if (dev < 0 || dev >= kNaMaxDevices) return TPC_E_ARG;
+    NaDevice nd;
+    if ((e = na_device(dev, nd)) != cudaSuccess) return cuda_fail(e);
+    if (n_tracks == 0) return TPC_OK;
+
+    MergePtrs m{};
+    m.tracks = dev_tracks; m.clusterIds = dev_cluster_ids;
+    m.counters = reinterpret_cast<const uint32_t*>(nd.scratch + kNaCounters);
+    m.mcount = reinterpret_cast<uint32_t*>(nd.scratch + kNaMCount);
+    m.key = reinterpret_cast<uint32_t*>(nd.scratch + kNaKey);
+    m.order = reinterpret_cast<uint32_t*>(nd.scratch + kNaOrder);
+    m.bestIn = reinterpret_cast<unsigned long long*>(nd.scratch + kNaBestIn);
+    m.out = reinterpret_cast<int32_t*>(nd.scratch + kNaOut);
+    m.outChi2 = reinterpret_cast<float*>(nd.scratch + kNaOutChi2);
+    m.binStart = reinterpret_cast<uint32_t*>(nd.scratch + kNaBinStart);
+    m.binCursor = reinterpret_cast<uint32_t*>(nd.scratch + kNaBinCursor);
+    m.next = dev_next; m.prev = dev_prev; m.chi2 = dev_chi2;
+    m.merged = nullptr; m.segments = nullptr;        // k7_chains is not part of this entry point: the links are the result
+    m.nBins = n_sectors * n_rows;
+    DevParams dp; dp.P = P; dp.CB = (float)(-0.299792458e-2 * (double)bz_tesla); dp.nSec = n_sectors; dp.nRows = n_rows;
+    const int perSide = n_sectors >= 36 ? 18 : n_sectors;
+    const float cosB = (float)std::cos((double)sector_dphi), sinB = (float)std::sin((double)sector_dphi);
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    const int grid = nd.blocks;
+    k7na_begin<<<1, 32, 0, s>>>(n_tracks);
+    k7_init<<<grid, kK7Threads, 0, s>>>(m, n_rows);        // clears the bins, the cursors, the best-partner words, the outputs
+    k7_hist<<<grid, kK7Threads, 0, s>>>(m, n_rows);
+    k7_scan<<<1, 1024, 0, s>>>(m);
+    k7_scatter<<<grid, kK7Threads, 0, s>>>(m, n_rows);
+    k7_match<<<grid, kK7Threads, 0, s>>>(m, dp, perSide, cosB, sinB);
+    k7_link<<<grid, kK7Threads, 0, s>>>(m);
+    if ((e = cudaGetLastError()) != cudaSuccess) return cuda_fail(e);
+    return TPC_OK;
+}
