@@ -309,7 +309,23 @@ def time_frame_leg(torch, binding, datagen, params, dev, reps: int = 3):
     trk.sync()
     st = trk.get_stats()
     trk.destroy()
-    return {"workload": "config4:timeframe-20x-central", "n_clusters": ev.n_clusters, "calls": reps, "ms_per_call": ms,
+    # the same time frame in slices of 9 sectors through a quarter of the workspace (tpc_track_event_sliced:
+    # synchronous, results of every slice downloaded - wall clock of the call, input resident on the device)
+    per_sector = ev.row_counts.reshape(ev.n_sectors, ev.n_rows).sum(axis=1)
+    fullest = max(int(per_sector[s:s + 9].sum()) for s in range(0, ev.n_sectors, 9))
+    trk = binding.Tracker(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz, params)
+    trk.set_stream(stream.cuda_stream)
+    ws_sl = trk.allocate_workspace(fullest, device=dev)
+    dy, dz = torch.from_numpy(ev.y).to(dev), torch.from_numpy(ev.z).to(dev)
+    trk.track_event_sliced(ev.row_counts, dy, dz, 9)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    tr_sl, _ = trk.track_event_sliced(ev.row_counts, dy, dz, 9)
+    sliced_ms = (time.perf_counter() - t0) * 1e3
+    trk.destroy()
+    sliced = {"sectors_per_slice": 9, "ms_per_call_wall_with_download": round(sliced_ms, 2), "n_tracks": int(tr_sl.size),
+              "workspace_bytes": int(ws_sl), "workspace_over_whole": round(ws_sl / ws, 3)}
+    return {"workload": "config4:timeframe-20x-central", "n_clusters": ev.n_clusters, "calls": reps, "ms_per_call": ms, "sliced": sliced,
             "value": ev.n_clusters / (ms * 1e-3), "unit": UNIT, "central_events_per_sec": 20.0 / (ms * 1e-3),
             "n_start_hits": st["n_start_hits"], "n_tracklet_hits": st["n_tracklet_hits"], "n_tracks": st["n_tracks"],
             "workspace_over_input": round(ws / (12.0 * ev.n_clusters), 2),

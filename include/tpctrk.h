@@ -251,6 +251,21 @@ int tpc_refit_tracks(tpc_tracker* t);
 /* Synchronise and download: refit[i] belongs to merged[i] of tpc_get_merged (same event).  Library-owned pinned memory. */
 int tpc_get_refit(tpc_tracker* t, const tpc_refit_track** refit, int32_t* n_merged);
 
+/* ---- Slicing ("If GPU memory would become insufficient, we can easily employ a slicing approach,
+ * processing parts of the time-frame one after another in a similar fashion as we currently process the TPC sectors") ----
+ * Phase I of a whole event (arguments as tpc_load_event: host or device pointers) in slices of sectors_per_slice
+ * consecutive sectors, one slice after the other through the SAME workspace, which therefore only has to hold the
+ * fullest slice: tpc_workspace_bytes(t, max over slices of the slice's clusters).  Sectors are independent in Phase I,
+ * so the result is the unsliced one: the same tracks (sector numbers of the whole event, event-global cluster ids),
+ * slice after slice.  Synchronous; the outputs are library-owned host memory, valid until the next sliced call or
+ * destroy.  Afterwards the tracker holds the LAST slice (tpc_get_stats, tpc_debug_dump, tpc_merge_tracks see that
+ * slice only; merging over all slices: upload the tracks and use tpc_merge_links_no_alloc, or run unsliced).
+ * Errors: TPC_E_ARG (null pointer, negative count, sectors_per_slice < 1), TPC_E_STATE (no workspace), TPC_E_NOMEM (a
+ * slice has more clusters than the workspace holds: checked before anything runs), TPC_E_OVERFLOW (a slice exceeded
+ * the tracklet capacity: enlarge the workspace or take fewer sectors per slice). */
+int tpc_track_event_sliced(tpc_tracker* t, const int32_t* row_counts, const float* y, const float* z, int32_t sectors_per_slice,
+                           const tpc_track** tracks, int32_t* n_tracks, const uint32_t** cluster_ids, int64_t* n_cluster_ids);
+
 /* ---- Track merging without any allocation (for callers that cannot call cudaMalloc: code under CUDA graph capture,
  * tight serving loops, harnesses that forbid it) ----
  * The K7 kernels of tpc_merge_tracks (same reading S7, same arithmetic, same links and chi2) with their scratch - the

@@ -100,6 +100,8 @@ def lib():
         L.tpc_track_sectors.argtypes = [vp]
         L.tpc_get_tracks.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(i32), ctypes.POINTER(vp), ctypes.POINTER(i64)]
         L.tpc_sync.argtypes = [vp]
+        L.tpc_track_event_sliced.argtypes = [vp, vp, vp, vp, i32, ctypes.POINTER(vp), ctypes.POINTER(i32), ctypes.POINTER(vp),
+                                             ctypes.POINTER(i64)]
         L.tpc_merge_tracks.argtypes = [vp]
         L.tpc_refit_tracks.argtypes = [vp]
         L.tpc_get_refit.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(i32)]
@@ -263,6 +265,20 @@ class Tracker:
         if copy:
             tracks, ids = tracks.copy(), ids.copy()
         return (tracks, ids, rc) if allow_overflow else (tracks, ids)
+
+    def track_event_sliced(self, row_counts, y, z, sectors_per_slice):
+        """tpc_track_event_sliced -> (tracks, cluster ids) of the whole event, processed slice after slice."""
+        rc = np.ascontiguousarray(row_counts, dtype=np.int32).reshape(-1)
+        assert rc.size == self.n_sectors * self.n_rows
+        tp, ip = ctypes.c_void_p(), ctypes.c_void_p()
+        nt, nc = ctypes.c_int32(), ctypes.c_int64()
+        self._check(self._L.tpc_track_event_sliced(self._h, rc.ctypes.data, _ptr(y), _ptr(z), int(sectors_per_slice), ctypes.byref(tp),
+                                                   ctypes.byref(nt), ctypes.byref(ip), ctypes.byref(nc)), "tpc_track_event_sliced")
+        tracks = np.frombuffer((ctypes.c_char * (nt.value * TRACK_DTYPE.itemsize)).from_address(tp.value), dtype=TRACK_DTYPE).copy() \
+            if nt.value else np.zeros(0, dtype=TRACK_DTYPE)
+        ids = np.frombuffer((ctypes.c_char * (nc.value * 4)).from_address(ip.value), dtype=np.uint32).copy() \
+            if nc.value else np.zeros(0, dtype=np.uint32)
+        return tracks, ids
 
     def merge_tracks(self):
         return self._check(self._L.tpc_merge_tracks(self._h), "tpc_merge_tracks")

@@ -89,6 +89,8 @@ struct tpc_tracker {
     int maxRowN = 0;                        // clusters in the fullest (sector,row) of the loaded event
     bool k2Stage = false;                   // tpc_set_neighbour_staging
 
+    std::vector<tpc_track> slTracks;        // tpc_track_event_sliced: the slices' results, concatenated
+    std::vector<uint32_t> slIds;
     // results (pinned)
     tpc_track* outTracks = nullptr; int64_t outTracksCap = 0;
     uint32_t* outIds = nullptr; int64_t outIdsCap = 0;
@@ -876,6 +878,53 @@ int tpc_get_tracks(tpc_tracker* t, const tpc_track** tracks, int32_t* n_tracks, 
     *tracks = t->outTracks; *n_tracks = (int32_t)nT; *cluster_ids = t->outIds; *n_cluster_ids = nC;
     t->fetched = true;
     return t->counters[kNStart] > (uint32_t)t->dev.maxTracklets ? TPC_E_OVERFLOW : TPC_OK;
+}
+
+// PAPER.md:107 slicing: the event's sectors in groups, one group after the other through the same workspace.
+int tpc_track_event_sliced(tpc_tracker* t, const int32_t* row_counts, const float* y, const float* z, int32_t sectors_per_slice,
+                           const tpc_track** tracks, int32_t* n_tracks, const uint32_t** cluster_ids, int64_t* n_cluster_ids) {
+    if (!t || !row_counts || !tracks || !n_tracks || !cluster_ids || !n_cluster_ids || sectors_per_slice < 1) return TPC_E_ARG;
+    if (!t->ws) return TPC_E_STATE;
+    std::vector<int64_t> secBase(t->nSec + 1, 0);     // clusters in front of each sector = its offset in y, z and in the ids
+    for (int s = 0; s < t->nSec; s++) {
+        int64_t n = 0;
+        for (int r = 0; r < t->nRows; r++) {
+            const int32_t c = row_counts[s * t->nRows + r];
+            if (c < 0) return TPC_E_ARG;
+            n += c;
+        }
+        secBase[s + 1] = secBase[s] + n;
+    }
+    if (secBase[t->nSec] > 0 && (!y || !z)) return TPC_E_ARG;
+    if (secBase[t->nSec] > 0xFFFFFFFFll) return TPC_E_ARG;                       // ids are 32-bit
+    for (int s0 = 0; s0 < t->nSec; s0 += sectors_per_slice)
+        if (secBase[std::min(t->nSec, s0 + sectors_per_slice)] - secBase[s0] > t->maxClusters) return TPC_E_NOMEM;
+    t->slTracks.clear(); t->slIds.clear();
+    std::vector<int32_t> counts(t->nRowsTotal);
+    for (int s0 = 0; s0 < t->nSec; s0 += sectors_per_slice) {
+        const int s1 = std::min(t->nSec, s0 + sectors_per_slice);
+        std::fill(counts.begin(), counts.end(), 0);
+        std::copy(row_counts + (size_t)s0 * t->nRows, row_counts + (size_t)s1 * t->nRows, counts.begin() + (size_t)s0 * t->nRows);
+        const int64_t base = secBase[s0];
+        int rc = tpc_load_event(t, counts.data(), y ? y + base : nullptr, z ? z + base : nullptr);
+        if (rc != TPC_OK) return rc;
+        if ((rc = tpc_track_sectors(t)) != TPC_OK) return rc;
+        const tpc_track* tr = nullptr; const uint32_t* ids = nullptr;
+        int32_t nT = 0; int64_t nC = 0;
+        if ((rc = tpc_get_tracks(t, &tr, &nT, &ids, &nC)) != TPC_OK) return rc;     // (waits for the slice: also for its input DMA)
+        const int64_t idOff = (int64_t)t->slIds.size();
+        if (idOff + nC > 0x7FFFFFFFll) return TPC_E_ARG;                         // cluster_offset is an int32
+        const size_t tOff = t->slTracks.size();
+        t->slTracks.resize(tOff + (size_t)nT);
+        t->slIds.resize((size_t)(idOff + nC));
+        if (nT) std::memcpy(t->slTracks.data() + tOff, tr, sizeof(tpc_track) * (size_t)nT);
+        for (int32_t i = 0; i < nT; i++) t->slTracks[tOff + i].cluster_offset += (int32_t)idOff;
+        uint32_t* dst = t->slIds.data() + idOff;
+        for (int64_t i = 0; i < nC; i++) dst[i] = ids[i] + (uint32_t)base;
+    }
+    *tracks = t->slTracks.data(); *n_tracks = (int32_t)t->slTracks.size();
+    *cluster_ids = t->slIds.data(); *n_cluster_ids = (int64_t)t->slIds.size();
+    return TPC_OK;
 }
 
 int tpc_get_stats(tpc_tracker* t, tpc_stats* out) {

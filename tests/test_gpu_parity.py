@@ -813,3 +813,67 @@ def test_final_fit_call_order_and_empty_event():
     trk, tracks, ids = run_gpu(empty, max_clusters=16)
     trk.merge_tracks(); trk.refit_tracks()
     assert trk.get_refit().size == 0
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Slicing: the event's sectors in groups through a workspace that only holds the fullest group
+
+def _canonical_tracks(tracks, ids):
+    """Tracks ordered by their first cluster id, each with its cluster list."""
+    key = ids[tracks["cluster_offset"]].astype(np.int64)
+    o = np.argsort(key)
+    t = tracks[o]
+    lists = [ids[a:a + n] for a, n in zip(t["cluster_offset"], t["n_clusters"])]
+    return t, lists
+
+
+@pytest.mark.parametrize("per_slice", [5, 18, 36, 1])
+def test_sliced_event_equals_the_whole_event(per_slice):
+    """tpc_track_event_sliced: same tracks (every field bit for bit), same event-global cluster ids as the unsliced
+    call - and as the oracle - with a workspace sized for the fullest slice only."""
+    _cuda()
+    ev = datagen.config_event(2, seed=4)
+    trk, tracks, ids = run_gpu(ev)
+    whole_ws = trk.get_stats()["workspace_bytes_used"]
+    per_sector = ev.row_counts.reshape(ev.n_sectors, ev.n_rows).sum(axis=1)
+    fullest = max(int(per_sector[s:s + per_slice].sum()) for s in range(0, ev.n_sectors, per_slice))
+    t2 = binding.Tracker(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz)
+    ws = t2.allocate_workspace(fullest)
+    if per_slice < 36:
+        assert fullest < ev.n_clusters and ws < whole_ws
+    for y, z in ((ev.y, ev.z), (__import__("torch").from_numpy(ev.y).cuda(), __import__("torch").from_numpy(ev.z).cuda())):
+        st, sids = t2.track_event_sliced(ev.row_counts, y, z, per_slice)
+        a, la = _canonical_tracks(tracks, ids)
+        b, lb = _canonical_tracks(st, sids)
+        assert a.size == b.size and a.size > 100
+        for f in a.dtype.names:
+            if f != "cluster_offset":
+                assert np.array_equal(a[f], b[f]), f
+        assert all(np.array_equal(p, q) for p, q in zip(la, lb))
+        assert np.all(np.diff(st["sector"] // per_slice) >= 0)          # slice after slice
+    assert t2.debug_check_guards() == 0
+    ref = oracle.run_event(ev)
+    assert np.array_equal(np.sort(sids.astype(np.int64)), np.sort(ref.cluster_ids.astype(np.int64)))
+
+
+def test_sliced_event_errors():
+    _cuda()
+    ev = datagen.config_event(1, seed=1)
+    per_sector = ev.row_counts.reshape(ev.n_sectors, ev.n_rows).sum(axis=1)
+    t2 = binding.Tracker(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz)
+    with pytest.raises(binding.TpcError) as e:
+        t2.track_event_sliced(ev.row_counts, ev.y, ev.z, 4)
+    assert e.value.code == binding.TPC_E_STATE
+    t2.allocate_workspace(int(per_sector.max()))                  # one sector at a time fits, two may not
+    t2.track_event_sliced(ev.row_counts, ev.y, ev.z, 1)
+    with pytest.raises(binding.TpcError) as e:
+        t2.track_event_sliced(ev.row_counts, ev.y, ev.z, 36)
+    assert e.value.code == binding.TPC_E_NOMEM
+    with pytest.raises(binding.TpcError) as e:
+        t2.track_event_sliced(ev.row_counts, ev.y, ev.z, 0)
+    assert e.value.code == binding.TPC_E_ARG
+    empty = datagen.event_from_hits([], 36, datagen.default_row_x(), 0.5)
+    t3 = binding.Tracker(36, empty.n_rows, empty.row_x, 0.5)
+    t3.allocate_workspace(16)
+    st, sids = t3.track_event_sliced(empty.row_counts, empty.y, empty.z, 7)
+    assert st.size == 0 and sids.size == 0
