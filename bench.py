@@ -281,6 +281,42 @@ def multi_event_leg(torch, binding, datagen, args, params, dev, rank: int, k: in
             "note": "k independent synthetic events (other seeds) as 36*k sectors of one tracker, one call"}
 
 
+def instances_leg(torch, binding, ev, params, dev, n_inst: int, n_events: int):
+    """PAPER.md:82-84 (several tracker instances share the GPU; the paper measures -24 % per event with two): n_inst
+    trackers on n_inst streams, inputs resident in HBM, ONE host thread issuing tpc_track_sectors round robin and
+    waiting for the oldest; wall clock per event.  Extra key, not the metric (no L2 flush: the instances' 0.4 GB
+    workspaces evict each other)."""
+    pipes = []
+    for _ in range(n_inst):
+        sti = torch.cuda.Stream(device=dev)
+        ti = binding.Tracker(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz, params)
+        ti.set_stream(sti.cuda_stream)
+        ti.allocate_workspace(ev.n_clusters, device=dev)
+        if n_inst > 1:
+            ti.set_dependent_launch(False)
+        ti.set_output_prefetch(False)
+        y, z = torch.from_numpy(ev.y).to(dev), torch.from_numpy(ev.z).to(dev)
+        ti.load_event(ev.row_counts, y, z)
+        pipes.append((ti, sti, y, z))
+
+    def run(n):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for i in range(n + n_inst):
+            ti = pipes[i % n_inst][0]
+            if i >= n_inst:
+                ti.sync()
+            if i < n:
+                ti.track_sectors()
+        torch.cuda.synchronize()
+        return (time.perf_counter() - t0) / n * 1e3
+    run(2 * n_inst)
+    ms = run(n_events)
+    for p_ in pipes:
+        p_[0].destroy()
+    return ms
+
+
 def time_frame_leg(torch, binding, datagen, params, dev, reps: int = 3):
     """BASELINE.json:configs[4] (extra key, not the headline): a Run-3-style time frame - 20 overlapped central events,
     ~31.6 M clusters - tracked by ONE tpc_track_sectors call (north_star).  Same timing rules as the main leg."""
@@ -592,6 +628,13 @@ def main():
         me = multi_event_leg(torch, binding, datagen, args, params, dev, rank, args.events_per_call, max(3, min(args.steps, 10)))
         me["value"] = reduce_over_ranks(dist, me["value"], "sum", dev)      # whole job: sum of the ranks' rates
         out["multi_event"] = me
+    if rank == 0 and args.events_per_call > 1 and args.config <= 3:
+        n_ev = max(12, min(4 * args.steps, 48))
+        one = instances_leg(torch, binding, ev, params, dev, 1, n_ev)
+        three = instances_leg(torch, binding, ev, params, dev, 3, n_ev // 3 * 3)
+        out["concurrent_instances"] = {"instances": 3, "ms_per_event": round(three, 4), "one_instance_ms_per_event": round(one, 4),
+                                       "value": ev.n_clusters / (three * 1e-3), "unit": UNIT,
+                                       "note": "PAPER.md:82-84: trackers on separate streams, inputs resident, no L2 flush, wall clock"}
     if rank == 0 and not args.no_time_frame and args.config == 3:
         del trk, y_dev, z_dev                            # (the time frame needs ~9 GB of workspace)
         out["time_frame"] = time_frame_leg(torch, binding, datagen, params, dev)

@@ -273,7 +273,13 @@ constexpr int kK2Threads = TPC_K2T;
 #ifndef TPC_K2CAP
 #define TPC_K2CAP 8
 #endif
-constexpr int kK2Cap = TPC_K2CAP;   // down-candidates cached per thread; beyond that a nested rescan (slow, exact)
+constexpr int kK2Cap = TPC_K2CAP;   // down-candidates cached per thread (registers); beyond that a grid query per up-candidate
+#ifndef TPC_K2CAPD
+#define TPC_K2CAPD 12
+#endif
+constexpr int kK2CapDense = TPC_K2CAPD;   // ... in the instantiation for dense rows (time frames: ~20x the candidates per window).
+// Measured (central event K2 us / time frame K2 ms), grid query on: cap 8: 83.7 / 7.2, 10: 88.6 / 6.6, 12: 95.5 / 6.4,
+// 16: 104.8 / 6.5; with the whole-window rescan it replaced, cap 8: 89.5 / 8.9
 #ifndef TPC_K2B
 #define TPC_K2B 8
 #endif
@@ -348,9 +354,25 @@ __device__ __forceinline__ void k2_for_window(const RowGrid& R, const K2Row& V, 
     }
 }
 
+// the same for a box given by its bounds (nothing if a bound pair is crossed)
+template <class F>
+__device__ __forceinline__ void k2_for_box(const RowGrid& R, const K2Row& V, float ylo, float yhi, float zlo, float zhi, F&& f) {
+    const int by0 = bin_of(ylo - kGridMargin, R.y0, R.invY, R.nY);
+    const int by1 = bin_of(yhi + kGridMargin, R.y0, R.invY, R.nY);
+    const int bz0 = bin_of(zlo - kGridMargin, R.z0, R.invZ, R.nZ);
+    const int bz1 = bin_of(zhi + kGridMargin, R.z0, R.invZ, R.nZ);
+    if (by0 > by1) return;
+    const uint32_t* __restrict__ bs = V.bs - V.bBase;
+    const float2* __restrict__ hs = V.hs - V.kBase;
+    for (int bz = bz0; bz <= bz1; bz++) {
+        const int k0 = (int)bs[bz * R.nY + by0], k1 = (int)bs[bz * R.nY + by1 + 1];
+        for (int k = k0; k < k1; k++) f(k, hs[k]);
+    }
+}
+
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
-template <bool kStage>
+template <bool kStage, int kCap>
 __global__ void __launch_bounds__(kK2Threads, TPC_K2B) k2_neighbours(DevPtrs d, DevParams dp) {
     __shared__ __align__(16) float2 sHitsU[kStage ? kK2StageHits : 1], sHitsD[kStage ? kK2StageHits : 1];
     __shared__ uint32_t sBinsU[kStage ? kK2StageBins : 1], sBinsD[kStage ? kK2StageBins : 1];
@@ -382,6 +404,8 @@ __global__ void __launch_bounds__(kK2Threads, TPC_K2B) k2_neighbours(DevPtrs d, 
     const float wu = -dxd / (dxu - dxd), wd = dxu / (dxu - dxd);
     const float wyU = dp.P.nf_ty * dxu + dp.P.nf_c, wzU = dp.P.nf_tz * dxu + dp.P.nf_c;
     const float wyD = dp.P.nf_ty * (-dxd) + dp.P.nf_c, wzD = dp.P.nf_tz * (-dxd) + dp.P.nf_c;
+    const float rwd = 1.0f / wd;
+    const float boxR = sqrtf(dp.P.nf_d2max) * rwd * 1.001f + 2.0e-3f;      // (see the rescan below)
     const uint32_t* __restrict__ origU = d.orig + Ru.hitOff;
     const uint32_t* __restrict__ origD = d.orig + Rd.hitOff;
     K2Row VU{d.hits + Ru.hitOff, d.binStart + Ru.binOff, 0, 0}, VD{d.hits + Rd.hitOff, d.binStart + Rd.binOff, 0, 0};
@@ -442,14 +466,14 @@ __global__ void __launch_bounds__(kK2Threads, TPC_K2B) k2_neighbours(DevPtrs d, 
 
     for (int i = i0 + threadIdx.x; i < i1; i += kK2Threads) {
         const float2 h = d.hits[R.hitOff + i];
-        float cy[kK2Cap], cz[kK2Cap];
-        int ck[kK2Cap];
+        float cy[kCap], cz[kCap];
+        int ck[kCap];
         int nd = 0;
         const WinRanges rD = k2_win_ranges(Rd, VD, h.x, h.y, wyD, wzD);
         const WinRanges rU = k2_win_ranges(Ru, VU, h.x, h.y, wyU, wzU);
         k2_scan(rD, Rd, VD, [&](int k, float2 c) {
             if (fabsf(c.x - h.x) <= wyD && fabsf(c.y - h.y) <= wzD) {
-                if (nd < kK2Cap) { cy[nd] = wd * c.x; cz[nd] = wd * c.y; ck[nd] = k; }
+                if (nd < kCap) { cy[nd] = wd * c.x; cz[nd] = wd * c.y; ck[nd] = k; }
                 nd++;
             }
         });
@@ -467,13 +491,21 @@ __global__ void __launch_bounds__(kK2Threads, TPC_K2B) k2_neighbours(DevPtrs d, 
             k2_scan(rU, Ru, VU, [&](int ku, float2 c) {
                 if (!(fabsf(c.x - h.x) <= wyU && fabsf(c.y - h.y) <= wzU)) return;
                 const float py = wu * c.x, pz = wu * c.y;
-                if (nd <= kK2Cap) {
+                if (nd <= kCap) {
                     for (int j = 0; j < nd; j++) {
                         const float ey = h.x - (py + cy[j]), ez = h.y - (pz + cz[j]);
                         consider(ku, ck[j], ey * ey + ez * ez);
                     }
                 } else {
-                    k2_for_window(Rd, VD, h.x, h.y, wyD, wzD, [&](int kd, float2 e) {
+                    // More down-candidates than the cache holds (dense rows: time frames).  A pair counts only if its
+                    // residual is <= nf_d2max, i.e. if the down-hit lies within sqrt(nf_d2max) / wd of the point that
+                    // this up-hit mirrors through h; so the down row's grid is asked for that box (with a margin far
+                    // above the rounding of the two expressions) instead of the whole window again: the pairs left
+                    // out are rejected whatever their order, the others are compared exactly as before.
+                    const float my = (h.x - py) * rwd, mz = (h.y - pz) * rwd;
+                    // (the box cut to the window: what a staged block holds of the row is what the window can reach)
+                    k2_for_box(Rd, VD, fmaxf(my - boxR, h.x - wyD), fminf(my + boxR, h.x + wyD), fmaxf(mz - boxR, h.y - wzD),
+                               fminf(mz + boxR, h.y + wzD), [&](int kd, float2 e) {
                         if (!(fabsf(e.x - h.x) <= wyD && fabsf(e.y - h.y) <= wzD)) return;
                         const float ey = h.x - (py + wd * e.x), ez = h.y - (pz + wd * e.y);
                         consider(ku, kd, ey * ey + ez * ez);

@@ -692,8 +692,11 @@ int tpc_track_sectors(tpc_tracker* t) {
         attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
         attr[0].val.programmaticStreamSerializationAllowed = 1;
         cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
-        if (t->k2Stage) CUDA_TRY(t, cudaLaunchKernelEx(&cfg, k2_neighbours<true>, d, dp));
-        else CUDA_TRY(t, cudaLaunchKernelEx(&cfg, k2_neighbours<false>, d, dp));
+        // dense rows (time frames; the same criterion as K3's start order below): more cached down-candidates per thread
+        const bool dense = t->nClusters > (int64_t)1000 * NR;
+        if (t->k2Stage) CUDA_TRY(t, cudaLaunchKernelEx(&cfg, k2_neighbours<true, kK2Cap>, d, dp));
+        else if (dense) CUDA_TRY(t, cudaLaunchKernelEx(&cfg, k2_neighbours<false, kK2CapDense>, d, dp));
+        else CUDA_TRY(t, cudaLaunchKernelEx(&cfg, k2_neighbours<false, kK2Cap>, d, dp));
     }
     if (timed) CUDA_TRY(t, cudaEventRecord(t->ev[2], s));
     CUDA_TRY(t, launch_dep(pdl, k3_clean_start, NR, kK3Threads, 0, s, d, dp, t->nClusters > (int64_t)1000 * NR ? 1 : 0));
