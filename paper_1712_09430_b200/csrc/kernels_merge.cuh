@@ -289,38 +289,55 @@ __global__ void __launch_bounds__(kK7Threads) k8_refit(MergePtrs m, DevPtrs d, D
         bool ok = kf_propagate(st, d.rowX[outer.last_row] - x, k8_field_cb(st, x, dp.CB, P.field_ar, P.field_az), P.kf_smax, nw);
         if (ok) st = nw;
         bool first = true;
-        for (int sg = M.n_segments - 1; ok && sg >= 0; sg--) {
-            const tpc_track seg = m.tracks[segs[sg]];
-            for (int c = seg.n_clusters - 1; ok && c >= 0; c--) {
-                const unsigned at = (unsigned)seg.cluster_offset + (unsigned)c;
-                const float2 h = d.hits[d.clusterPos[at]];
-                const float xr = d.rowX[d.clusterRow[at]];
-                if (first) {           // the outermost cluster is the starting point, not a measurement
-                    st.p0 = h.x; st.p1 = h.y; x = xr;
-                    kf_init_cov(st, P);
-                    chi2 = 0.f; nfit = 0;
-                    first = false;
-                    continue;
-                }
-                if (seg.sector != curSector) {       // into the next segment's sector frame
-                    int dsec = seg.sector % perSide - curSector % perSide;
-                    if (dsec > perSide / 2) dsec -= perSide;
-                    if (dsec < -perSide / 2) dsec += perSide;
-                    ok = k7_rotate(st, x, cosB, dsec > 0 ? sinB : -sinB, k8_field_cb(st, x, dp.CB, P.field_ar, P.field_az), P.kf_smax);
-                    curSector = seg.sector;
-                    if (!ok) break;
-                }
-                const float x0 = x, y0 = st.p0, z0 = st.p1;
-                ok = kf_propagate(st, xr - x, k8_field_cb(st, x, dp.CB, P.field_ar, P.field_az), P.kf_smax, nw);
-                if (!ok) break;
-                st = nw; x = xr;
-                if (P.ms_x0_inv > 0.f) {
-                    const float dx = x - x0, dy = st.p0 - y0, dz = st.p1 - z0;
-                    k8_scatter(st, sqrtf((dx * dx + dy * dy) + dz * dz), P.ms_x0_inv);
-                }
-                kf_update_hit(st, h.x, h.y, P.err2_y, P.err2_z, chi2, true);
-                nfit++;
+        // The clusters of the merged track, outermost first: segment after segment inward, each from its last cluster to
+        // its first.  The pass is a chain of dependent steps, so what a step reads is requested ahead of it: the
+        // cluster's sorted position and pad row two steps ahead (qPos, qRow), its coordinates and the row's x one step
+        // ahead (nH, nX) - otherwise every step would wait for two dependent memory round trips.
+        const int nSteps = M.n_clusters;          // = sum of the segments' clusters (k7_chains)
+        int qSg = M.n_segments - 1, qOff = outer.cluster_offset, qC = outer.n_clusters - 1, qSector = outer.sector;
+        auto q_next = [&]() {                     // the cursor moves one cluster inward
+            if (qC > 0) { qC--; return; }
+            qSg--;
+            const tpc_track* tn = m.tracks + segs[qSg];
+            qOff = tn->cluster_offset; qC = tn->n_clusters - 1; qSector = tn->sector;
+        };
+        uint32_t qPos = d.clusterPos[(unsigned)qOff + (unsigned)qC];
+        int qRow = d.clusterRow[(unsigned)qOff + (unsigned)qC], qSec = qSector;
+        float2 nH = d.hits[qPos];
+        float nX = d.rowX[qRow];
+        int nSec = qSec;
+        if (nSteps > 1) { q_next(); qPos = d.clusterPos[(unsigned)qOff + (unsigned)qC]; qRow = d.clusterRow[(unsigned)qOff + (unsigned)qC]; qSec = qSector; }
+        for (int k = 0; ok && k < nSteps; k++) {
+            const float2 h = nH;
+            const float xr = nX;
+            const int sec = nSec;
+            if (k + 1 < nSteps) { nH = d.hits[qPos]; nX = d.rowX[qRow]; nSec = qSec; }
+            if (k + 2 < nSteps) { q_next(); qPos = d.clusterPos[(unsigned)qOff + (unsigned)qC]; qRow = d.clusterRow[(unsigned)qOff + (unsigned)qC]; qSec = qSector; }
+            if (first) {           // the outermost cluster is the starting point, not a measurement
+                st.p0 = h.x; st.p1 = h.y; x = xr;
+                kf_init_cov(st, P);
+                chi2 = 0.f; nfit = 0;
+                first = false;
+                continue;
             }
+            if (sec != curSector) {       // into the next segment's sector frame
+                int dsec = sec % perSide - curSector % perSide;
+                if (dsec > perSide / 2) dsec -= perSide;
+                if (dsec < -perSide / 2) dsec += perSide;
+                ok = k7_rotate(st, x, cosB, dsec > 0 ? sinB : -sinB, k8_field_cb(st, x, dp.CB, P.field_ar, P.field_az), P.kf_smax);
+                curSector = sec;
+                if (!ok) break;
+            }
+            const float x0 = x, y0 = st.p0, z0 = st.p1;
+            ok = kf_propagate(st, xr - x, k8_field_cb(st, x, dp.CB, P.field_ar, P.field_az), P.kf_smax, nw);
+            if (!ok) break;
+            st = nw; x = xr;
+            if (P.ms_x0_inv > 0.f) {
+                const float dx = x - x0, dy = st.p0 - y0, dz = st.p1 - z0;
+                k8_scatter(st, sqrtf((dx * dx + dy * dy) + dz * dz), P.ms_x0_inv);
+            }
+            kf_update_hit(st, h.x, h.y, P.err2_y, P.err2_z, chi2, true);
+            nfit++;
         }
         tpc_refit_track r;
         r.first_track = segs[0];
