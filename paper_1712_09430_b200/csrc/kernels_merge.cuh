@@ -118,35 +118,37 @@ __device__ __forceinline__ bool k7_rotate(KFState& a, float& x, float cb, float 
 }
 
 // chi2 = d^T S^-1 d by LDL^T without pivoting (S symmetric 5x5, lower triangle s[15]); 1e30 if a pivot is not positive.
-__device__ __forceinline__ float k7_chi2(const float d[5], const float s[15]) {
+// The forward substitution w = L^-1 d runs along with the factorisation (row j needs the columns < j only), term by term
+// in the order of the definition: chi2 = sum_j w_j^2 / D_j.  Every term is >= 0 while the pivots are positive, so the
+// partial sums never fall: as soon as one exceeds `cap` (the caller rejects chi2 > cap) or a pivot fails, the
+// candidate's fate is decided and the rest is skipped - most candidates are strangers and leave at the first term.
+// A returned value <= cap is the full sum.
+__device__ __forceinline__ float k7_chi2(const float d[5], const float s[15], float cap) {
     float L[5][5], D[5], w[5];
     auto S = [&](int i, int j) { return s[i * (i + 1) / 2 + j]; };      // i >= j
-    bool bad = false;
+    float chi = 0.f;
 #pragma unroll
     for (int j = 0; j < 5; j++) {
         float dj = S(j, j);
 #pragma unroll
         for (int q = 0; q < j; q++) dj = dj - (L[j][q] * L[j][q]) * D[q];
-        bad = bad || !(dj > 0.f);
+        if (!(dj > 0.f)) return 1e30f;
         D[j] = dj;
+        float v = d[j];
+#pragma unroll
+        for (int q = 0; q < j; q++) v = v - L[j][q] * w[q];
+        w[j] = v;
+        chi = chi + (v * v) / dj;
+        if (!(chi <= cap)) return chi;
 #pragma unroll
         for (int i = j + 1; i < 5; i++) {
-            float v = S(i, j);
+            float u = S(i, j);
 #pragma unroll
-            for (int q = 0; q < j; q++) v = v - (L[i][q] * L[j][q]) * D[q];
-            L[i][j] = v / dj;
+            for (int q = 0; q < j; q++) u = u - (L[i][q] * L[j][q]) * D[q];
+            L[i][j] = u / dj;
         }
     }
-    float chi = 0.f;
-#pragma unroll
-    for (int i = 0; i < 5; i++) {
-        float v = d[i];
-#pragma unroll
-        for (int q = 0; q < i; q++) v = v - L[i][q] * w[q];
-        w[i] = v;
-        chi = chi + (v * v) / D[i];
-    }
-    return bad ? 1e30f : chi;
+    return chi;
 }
 
 __device__ __forceinline__ unsigned long long k7_pack(float chi2, uint32_t key) {
@@ -202,7 +204,7 @@ __global__ void __launch_bounds__(kK7Threads) k7_match(MergePtrs m, DevParams dp
                     const float s[15] = {o.c0 + TB.c[0], o.c1 + TB.c[1], o.c2 + TB.c[2], o.c3 + TB.c[3], o.c4 + TB.c[4],
                                          o.c5 + TB.c[5], o.c6 + TB.c[6], o.c7 + TB.c[7], o.c8 + TB.c[8], o.c9 + TB.c[9],
                                          o.c10 + TB.c[10], o.c11 + TB.c[11], o.c12 + TB.c[12], o.c13 + TB.c[13], o.c14 + TB.c[14]};
-                    const float c = k7_chi2(d, s);
+                    const float c = k7_chi2(d, s, dp.P.merge_chi2);
                     if (!(c <= dp.P.merge_chi2)) continue;
                     const uint32_t keyB = m.key[b];
                     if (best < 0 || c < bestC || (c == bestC && keyB < bestKey)) { best = (int)b; bestC = c; bestKey = keyB; }
