@@ -412,7 +412,7 @@ def main():
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--e2e-instances", type=int, default=3, help="tracker instances (streams) the ONE host thread of the end-to-end leg keeps in flight")
+    ap.add_argument("--e2e-instances", type=int, default=4, help="tracker instances (streams) the ONE host thread of the end-to-end leg keeps in flight")
     ap.add_argument("--neighbour-staging", action="store_true", help="K2 with its neighbour rows staged in shared memory (tpc_set_neighbour_staging; slower, for the ncu comparison)")
     ap.add_argument("--no-time-frame", action="store_true", help="skip the configs[4] leg (20 overlapped central events in one call)")
     ap.add_argument("--ncu-summary", default=None, metavar="REPORT.ncu-rep",
@@ -631,8 +631,9 @@ def main():
     if rank == 0 and args.events_per_call > 1 and args.config <= 3:
         n_ev = max(12, min(4 * args.steps, 48))
         one = instances_leg(torch, binding, ev, params, dev, 1, n_ev)
-        three = instances_leg(torch, binding, ev, params, dev, 3, n_ev // 3 * 3)
-        out["concurrent_instances"] = {"instances": 3, "ms_per_event": round(three, 4), "one_instance_ms_per_event": round(one, 4),
+        n_inst = max(2, args.e2e_instances)
+        three = instances_leg(torch, binding, ev, params, dev, n_inst, n_ev // n_inst * n_inst)
+        out["concurrent_instances"] = {"instances": n_inst, "ms_per_event": round(three, 4), "one_instance_ms_per_event": round(one, 4),
                                        "value": ev.n_clusters / (three * 1e-3), "unit": UNIT,
                                        "note": "PAPER.md:82-84: trackers on separate streams, inputs resident, no L2 flush, wall clock"}
     if rank == 0 and not args.no_time_frame and args.config == 3:
