@@ -47,12 +47,14 @@ __global__ void __launch_bounds__(kK7Threads) k7_init(MergePtrs m, int nRows) {
     }
 }
 __global__ void __launch_bounds__(kK7Threads) k7_hist(MergePtrs m, int nRows) {
+    grid_dep_wait();
     const unsigned nT = m.counters[kNTracks];
     for (unsigned t = blockIdx.x * kK7Threads + threadIdx.x; t < nT; t += gridDim.x * kK7Threads)
         atomicAdd(&m.binStart[m.tracks[t].sector * nRows + m.tracks[t].first_row], 1u);
 }
 // exclusive prefix of binStart[0..nBins] in place (one block; nBins is a few thousand)
 __global__ void __launch_bounds__(1024) k7_scan(MergePtrs m) {
+    grid_dep_wait();
     __shared__ uint32_t warpSum[32];
     __shared__ uint32_t carry;
     if (threadIdx.x == 0) carry = 0u;
@@ -78,6 +80,7 @@ __global__ void __launch_bounds__(1024) k7_scan(MergePtrs m) {
     if (threadIdx.x == 0) m.binStart[m.nBins + 1] = carry;
 }
 __global__ void __launch_bounds__(kK7Threads) k7_scatter(MergePtrs m, int nRows) {
+    grid_dep_wait();
     const unsigned nT = m.counters[kNTracks];
     for (unsigned t = blockIdx.x * kK7Threads + threadIdx.x; t < nT; t += gridDim.x * kK7Threads) {
         const int b = m.tracks[t].sector * nRows + m.tracks[t].first_row;
@@ -158,6 +161,7 @@ __device__ __forceinline__ unsigned long long k7_pack(float chi2, uint32_t key) 
 // One WARP per segment A (its candidates - a few to a few dozen - are shared out over the lanes): A's best outer
 // partner, and A's bid for being the best inner partner of every match.
 __global__ void __launch_bounds__(kK7Threads) k7_match(MergePtrs m, DevParams dp, int perSide, float cosB, float sinB) {
+    grid_dep_wait();
     const unsigned nT = m.counters[kNTracks];
     const int nRows = dp.nRows;
     const unsigned lane = threadIdx.x & 31u;
@@ -229,6 +233,7 @@ __global__ void __launch_bounds__(kK7Threads) k7_match(MergePtrs m, DevParams dp
 }
 // A link survives if it is mutual.
 __global__ void __launch_bounds__(kK7Threads) k7_link(MergePtrs m) {
+    grid_dep_wait();
     const unsigned nT = m.counters[kNTracks];
     for (unsigned a = blockIdx.x * kK7Threads + threadIdx.x; a < nT; a += gridDim.x * kK7Threads) {
         const int b = m.out[a];
@@ -237,6 +242,7 @@ __global__ void __launch_bounds__(kK7Threads) k7_link(MergePtrs m) {
 }
 // Merged tracks: one per segment without inner partner, its chain written out.
 __global__ void __launch_bounds__(kK7Threads) k7_chains(MergePtrs m) {
+    grid_dep_wait();
     const unsigned nT = m.counters[kNTracks];
     for (unsigned h = blockIdx.x * kK7Threads + threadIdx.x; h < nT; h += gridDim.x * kK7Threads) {
         if (m.prev[h] >= 0) continue;

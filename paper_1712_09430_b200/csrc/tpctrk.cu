@@ -737,13 +737,16 @@ int tpc_merge_tracks(tpc_tracker* t) {
     const float cosB = (float)std::cos((double)t->sectorDphi), sinB = (float)std::sin((double)t->sectorDphi);
     const int grid = t->k6Blocks;                            // grid-stride over the tracks (their number is on the device)
     CUDA_TRY(t, cudaEventRecord(t->evM0, s));
+    // the six kernels behind k7_init as programmatic dependents of the one before (each waits for it first thing:
+    // what is saved is the launch gap, ~2 us each), unless the tracker shares the GPU (tpc_set_dependent_launch)
+    const bool pdl = TPC_PDL && t->dependentLaunch;
     k7_init<<<grid, kK7Threads, 0, s>>>(m, t->nRows);
-    k7_hist<<<grid, kK7Threads, 0, s>>>(m, t->nRows);
-    k7_scan<<<1, 1024, 0, s>>>(m);
-    k7_scatter<<<grid, kK7Threads, 0, s>>>(m, t->nRows);
-    k7_match<<<grid, kK7Threads, 0, s>>>(m, dp, perSide, cosB, sinB);
-    k7_link<<<grid, kK7Threads, 0, s>>>(m);
-    k7_chains<<<grid, kK7Threads, 0, s>>>(m);
+    CUDA_TRY(t, launch_dep(pdl, k7_hist, grid, kK7Threads, 0, s, m, t->nRows));
+    CUDA_TRY(t, launch_dep(pdl, k7_scan, 1, 1024, 0, s, m));
+    CUDA_TRY(t, launch_dep(pdl, k7_scatter, grid, kK7Threads, 0, s, m, t->nRows));
+    CUDA_TRY(t, launch_dep(pdl, k7_match, grid, kK7Threads, 0, s, m, dp, perSide, cosB, sinB));
+    CUDA_TRY(t, launch_dep(pdl, k7_link, grid, kK7Threads, 0, s, m));
+    CUDA_TRY(t, launch_dep(pdl, k7_chains, grid, kK7Threads, 0, s, m));
     CUDA_TRY(t, cudaEventRecord(t->evM1, s));
     CUDA_TRY(t, cudaGetLastError());
     t->merged = true; t->mergeFetched = false; t->refitted = false; t->refitFetched = false;
