@@ -758,6 +758,8 @@ template <class T> static void update_c(double *p, double *c, double *chi2, int 
 
 #define DISPATCH(h, expr) ((h)->useDouble ? ((h)->d->expr) : ((h)->f->expr))
 
+/* memcpy for the getters: an empty std::vector may hand out a null data() pointer, which memcpy must not be given */
+static inline void copy_out(void *dst, const void *src, size_t bytes) { if (bytes) std::memcpy(dst, src, bytes); }
 extern "C" {
 
 void oracle_default_params(ParamsD *p) {
@@ -792,20 +794,20 @@ void oracle_get_links(void *hv, int which, int32_t *dst) {
     Handle *h = (Handle *)hv;
     auto cp = [&](auto &t) {
         const std::vector<int32_t> *v = which == 0 ? &t.linkUp : which == 1 ? &t.linkDn : which == 2 ? &t.linkUpC : &t.linkDnC;
-        std::memcpy(dst, v->data(), v->size() * sizeof(int32_t));
+        copy_out(dst, v->data(), v->size() * sizeof(int32_t));
     };
     if (h->useDouble) cp(*h->d); else cp(*h->f);
 }
 void oracle_get_tie_flags(void *hv, uint8_t *dst) {
     Handle *h = (Handle *)hv;
-    if (h->useDouble) std::memcpy(dst, h->d->tieS2.data(), h->d->tieS2.size());
-    else std::memcpy(dst, h->f->tieS2.data(), h->f->tieS2.size());
+    if (h->useDouble) copy_out(dst, h->d->tieS2.data(), h->d->tieS2.size());
+    else copy_out(dst, h->f->tieS2.data(), h->f->tieS2.size());
 }
 int64_t oracle_n_start_hits(void *hv) { Handle *h = (Handle *)hv; return (int64_t)DISPATCH(h, startHits.size()); }
 void oracle_get_start_hits(void *hv, int64_t *dst) {
     Handle *h = (Handle *)hv;
-    if (h->useDouble) std::memcpy(dst, h->d->startHits.data(), h->d->startHits.size() * 8);
-    else std::memcpy(dst, h->f->startHits.data(), h->f->startHits.size() * 8);
+    if (h->useDouble) copy_out(dst, h->d->startHits.data(), h->d->startHits.size() * 8);
+    else copy_out(dst, h->f->startHits.data(), h->f->startHits.size() * 8);
 }
 int64_t oracle_n_tracklets(void *hv) { Handle *h = (Handle *)hv; return (int64_t)DISPATCH(h, tracklets.size()); }
 int32_t oracle_sizeof_tracklet(void) { return (int32_t)sizeof(TrackletOut); }
@@ -813,29 +815,29 @@ int32_t oracle_sizeof_track(void) { return (int32_t)sizeof(TrackOut); }
 void oracle_get_tracklets(void *hv, void *dst, int32_t *row_hit) {
     Handle *h = (Handle *)hv;
     auto cp = [&](auto &t) {
-        std::memcpy(dst, t.tracklets.data(), t.tracklets.size() * sizeof(TrackletOut));
-        std::memcpy(row_hit, t.rowHit.data(), t.rowHit.size() * sizeof(int32_t));
+        copy_out(dst, t.tracklets.data(), t.tracklets.size() * sizeof(TrackletOut));
+        copy_out(row_hit, t.rowHit.data(), t.rowHit.size() * sizeof(int32_t));
     };
     if (h->useDouble) cp(*h->d); else cp(*h->f);
 }
 void oracle_get_owners(void *hv, int64_t *dst) {
     Handle *h = (Handle *)hv;
-    if (h->useDouble) std::memcpy(dst, h->d->owner.data(), h->d->owner.size() * 8);
-    else std::memcpy(dst, h->f->owner.data(), h->f->owner.size() * 8);
+    if (h->useDouble) copy_out(dst, h->d->owner.data(), h->d->owner.size() * 8);
+    else copy_out(dst, h->f->owner.data(), h->f->owner.size() * 8);
 }
 int64_t oracle_n_tracks(void *hv) { Handle *h = (Handle *)hv; return (int64_t)DISPATCH(h, tracks.size()); }
 int64_t oracle_n_cluster_ids(void *hv) { Handle *h = (Handle *)hv; return (int64_t)DISPATCH(h, clusterIds.size()); }
 void oracle_get_tracks(void *hv, void *dst, int32_t *cluster_ids) {
     Handle *h = (Handle *)hv;
     auto cp = [&](auto &t) {
-        std::memcpy(dst, t.tracks.data(), t.tracks.size() * sizeof(TrackOut));
-        std::memcpy(cluster_ids, t.clusterIds.data(), t.clusterIds.size() * sizeof(int32_t));
+        copy_out(dst, t.tracks.data(), t.tracks.size() * sizeof(TrackOut));
+        copy_out(cluster_ids, t.clusterIds.data(), t.clusterIds.size() * sizeof(int32_t));
     };
     if (h->useDouble) cp(*h->d); else cp(*h->f);
 }
 void oracle_get_stage_seconds(void *hv, double *dst) {
     Handle *h = (Handle *)hv;
-    std::memcpy(dst, h->useDouble ? h->d->stageSec : h->f->stageSec, 6 * sizeof(double));
+    copy_out(dst, h->useDouble ? h->d->stageSec : h->f->stageSec, 6 * sizeof(double));
 }
 
 /* ---- Phase II (S7): run after oracle_run; results indexed like the tracks of oracle_get_tracks ---- */
@@ -845,10 +847,10 @@ void oracle_get_merge(void *hv, int32_t *next, int32_t *prev, double *chi2, uint
     Handle *h = (Handle *)hv;
     auto cp = [&](auto &t) {
         const size_t n = t.mergeNext.size();
-        std::memcpy(next, t.mergeNext.data(), n * 4); std::memcpy(prev, t.mergePrev.data(), n * 4);
-        std::memcpy(chi2, t.mergeChi2.data(), n * 8); std::memcpy(tie, t.mergeTie.data(), n);
-        std::memcpy(merged_offset, t.mergedOffset.data(), t.mergedOffset.size() * 4);
-        std::memcpy(merged_segs, t.mergedSegs.data(), t.mergedSegs.size() * 4);
+        copy_out(next, t.mergeNext.data(), n * 4); copy_out(prev, t.mergePrev.data(), n * 4);
+        copy_out(chi2, t.mergeChi2.data(), n * 8); copy_out(tie, t.mergeTie.data(), n);
+        copy_out(merged_offset, t.mergedOffset.data(), t.mergedOffset.size() * 4);
+        copy_out(merged_segs, t.mergedSegs.data(), t.mergedSegs.size() * 4);
     };
     if (h->useDouble) cp(*h->d); else cp(*h->f);
 }
@@ -867,8 +869,8 @@ void oracle_refit(void *hv) { Handle *h = (Handle *)hv; if (h->useDouble) h->d->
 int32_t oracle_sizeof_refit(void) { return (int32_t)sizeof(Tracker<float>::RefitOut); }
 void oracle_get_refits(void *hv, void *dst) {
     Handle *h = (Handle *)hv;
-    if (h->useDouble) std::memcpy(dst, h->d->refits.data(), h->d->refits.size() * sizeof(Tracker<double>::RefitOut));
-    else std::memcpy(dst, h->f->refits.data(), h->f->refits.size() * sizeof(Tracker<float>::RefitOut));
+    if (h->useDouble) copy_out(dst, h->d->refits.data(), h->d->refits.size() * sizeof(Tracker<double>::RefitOut));
+    else copy_out(dst, h->f->refits.data(), h->f->refits.size() * sizeof(Tracker<float>::RefitOut));
 }
 /* primitives for the pins: rotate a state (x[1], p[5], c[15]) by beta; chi2 of d with covariance S (15) */
 int oracle_rotate(int use_double, double *x, double *p, double *c, double beta, double CB, double smax) {
