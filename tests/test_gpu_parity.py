@@ -916,7 +916,7 @@ def test_random_parameters_and_seeds_through_all_stages(capsys):
 def test_random_geometries_fields_and_events_per_call():
     """Other pad-row counts and pitches, field strengths of both signs, several events per call (the free-running K5
     kernel) and time-frame-like z shifts, each through every stage, merging, final fit, the sliced call and the
-    no-allocation merging entry (a fixed sample of a sweep that ran 344 such cases without a difference)."""
+    no-allocation merging entry (a fixed sample of sweeps that ran 1,154 such cases without a difference)."""
     torch = _cuda()
     rng = np.random.default_rng(77)
     for nrows, k_ev, n_events in ((64, 1, 1), (20, 2, 4), (200, 1, 2), (7, 5, 1), (159, 5, 1), (159, 2, 4)):
