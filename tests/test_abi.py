@@ -117,3 +117,22 @@ def test_no_cpu_fallback_in_product_path():
         t = binding.Tracker(1, 159, np.linspace(85, 246, 159).astype(np.float32), 0.5)
         with pytest.raises(RuntimeError):
             t.allocate_workspace(1000)
+
+
+def test_header_is_plain_c():
+    """include/tpctrk.h is a C header (C99, no torch or CUDA types): it compiles on its own with gcc and with g++."""
+    import subprocess
+    hdr = os.path.join(ROOT, "include", "tpctrk.h")
+    subprocess.check_call(["gcc", "-x", "c", "-std=c99", "-Wall", "-Wextra", "-pedantic", "-Werror", "-fsyntax-only", hdr])
+    subprocess.check_call(["g++", "-x", "c++", "-std=c++17", "-Wall", "-Werror", "-fsyntax-only", hdr])
+    # a C caller links against the library without any C++ or CUDA header
+    src = '#include "tpctrk.h"\nint main(void) { tpc_params p; tpc_default_params(&p); return p.min_hits == 10 ? 0 : 1; }\n'
+    import tempfile
+    with tempfile.TemporaryDirectory() as d:
+        c = os.path.join(d, "t.c")
+        open(c, "w").write(src)
+        exe = os.path.join(d, "t")
+        libdir = os.path.dirname(binding.library_path())
+        subprocess.check_call(["gcc", "-std=c99", "-I", os.path.join(ROOT, "include"), c, "-o", exe, "-L", libdir, "-ltpctrk",
+                               "-Wl,-rpath," + libdir])
+        assert subprocess.run([exe]).returncode == 0
