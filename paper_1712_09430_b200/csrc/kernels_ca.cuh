@@ -18,7 +18,8 @@ __device__ __forceinline__ int bin_of(float v, float v0, float inv, int n) {
 // One block per (sector,row): bounding box -> grid -> histogram in shared memory -> scan -> scatter.
 // Input: SoA y[], z[] as loaded (coalesced reads).  Output: sorted float2 (y,z), orig[], binStart[], grid.
 #ifndef TPC_ZF
-#define TPC_ZF 2.4f   /* measured on config 3 (K5 us): 1.5 -> 847, 1.8 -> 590, 2.2 -> 497, 2.6 -> 509; the steep side is the low one */
+#define TPC_ZF 2.1f   /* measured on config 3 (K5 us), 3 bins per hit: 1.5 -> 847, 1.8 -> 590, 2.2 -> 497, 2.6 -> 509; 2 bins per hit:
+                         1.9 -> 368, 2.0 -> 361, 2.1 -> 362, 2.2 -> 363, 2.3 -> 366, 2.4 -> 368, 2.7 -> 372; the steep side is the low one */
 #endif
 #ifndef TPC_K1T
 #define TPC_K1T 192
