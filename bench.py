@@ -292,8 +292,6 @@ def instances_leg(torch, binding, ev, params, dev, n_inst: int, n_events: int):
         ti = binding.Tracker(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz, params)
         ti.set_stream(sti.cuda_stream)
         ti.allocate_workspace(ev.n_clusters, device=dev)
-        if n_inst > 1:
-            ti.set_dependent_launch(False)
         ti.set_output_prefetch(False)
         y, z = torch.from_numpy(ev.y).to(dev), torch.from_numpy(ev.z).to(dev)
         ti.load_event(ev.row_counts, y, z)
@@ -412,7 +410,7 @@ def main():
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--e2e-instances", type=int, default=4, help="tracker instances (streams) the ONE host thread of the end-to-end leg keeps in flight")
+    ap.add_argument("--e2e-instances", type=int, default=6, help="tracker instances (streams) the ONE host thread of the end-to-end leg keeps in flight")
     ap.add_argument("--neighbour-staging", action="store_true", help="K2 with its neighbour rows staged in shared memory (tpc_set_neighbour_staging; slower, for the ncu comparison)")
     ap.add_argument("--no-time-frame", action="store_true", help="skip the configs[4] leg (20 overlapped central events in one call)")
     ap.add_argument("--ncu-summary", default=None, metavar="REPORT.ncu-rep",
@@ -534,8 +532,6 @@ def main():
         ti = binding.Tracker(ev.n_sectors, ev.n_rows, ev.row_x, ev.bz, params)
         ti.set_stream(sti.cuda_stream)
         ti.allocate_workspace(ev.n_clusters, device=dev)
-        if n_pipe > 1:
-            ti.set_dependent_launch(False)     # several trackers on concurrent streams: ordinary launches (tpctrk.h)
         pipes.append((ti, sti, torch.from_numpy(ev.y.copy()).pin_memory(), torch.from_numpy(ev.z.copy()).pin_memory()))
     last = [None]
 

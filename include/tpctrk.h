@@ -142,9 +142,9 @@ int tpc_set_stream(tpc_tracker* t, void* cuda_stream);
 int tpc_set_kernel_timing(tpc_tracker* t, int on);
 
 /* on != 0 (default): K2..K6 are launched as programmatic dependents of the kernel before them (only possible while
- * the kernel timing is off).  Best for a tracker that has the GPU to itself (-15 us per central event).  With several
- * trackers on concurrent streams (copies of one event behind the kernels of another) ordinary launches interleave
- * better: measured 0.73 vs 0.87 ms per event with four trackers in flight; switch it off there. */
+ * the kernel timing is off): -15 us per central event for a tracker that has the GPU to itself.  With several
+ * trackers on concurrent streams it makes little difference either way (end to end, one host thread: 0.51 vs 0.51 ms
+ * per event with six trackers in flight, 0.51 vs 0.55 with four). */
 int tpc_set_dependent_launch(tpc_tracker* t, int on);
 
 /* on != 0: the neighbours finder (K2) stages the pieces of the two adjacent pad rows that a block's hits can reach
