@@ -22,7 +22,7 @@ __device__ __forceinline__ int bin_of(float v, float v0, float inv, int n) {
                          1.9 -> 368, 2.0 -> 361, 2.1 -> 362, 2.2 -> 363, 2.3 -> 366, 2.4 -> 368, 2.7 -> 372; the steep side is the low one */
 #endif
 #ifndef TPC_K1T
-#define TPC_K1T 192
+#define TPC_K1T 160   /* threads per (sector,row) block; K1 us on config 3: 64 -> 53.5, 96 -> 49.6, 128 -> 45.6, 160 -> 44.0, 192 -> 47.6, 256 -> 51.7 */
 #endif
 constexpr int kK1Threads = TPC_K1T;
 constexpr int kK1Stage = 512;     // 8 KB of static shared memory beside the <= 32 KB dynamic histogram (48 KB limit)
