@@ -122,6 +122,7 @@ def test_no_cpu_fallback_in_product_path():
 def test_header_is_plain_c():
     """include/tpctrk.h is a C header (C99, no torch or CUDA types): it compiles on its own with gcc and with g++."""
     import subprocess
+    binding.lib()                                   # (builds the library if this test is the first to need it)
     hdr = os.path.join(ROOT, "include", "tpctrk.h")
     subprocess.check_call(["gcc", "-x", "c", "-std=c99", "-Wall", "-Wextra", "-pedantic", "-Werror", "-fsyntax-only", hdr])
     subprocess.check_call(["g++", "-x", "c++", "-std=c++17", "-Wall", "-Werror", "-fsyntax-only", hdr])
